@@ -1,0 +1,149 @@
+/* hsg.h — C ABI of the B200 Heisenberg-spin-glass Monte Carlo engine.
+ *
+ * One data-parallel hot path of Yavors'kii & Weigel, "Optimized GPU simulation of continuous-spin
+ * glass models" (arXiv 1204.6192; citations are /root/reference/PAPER.md line numbers): Monte Carlo
+ * sweeps of the 3D Edwards-Anderson Heisenberg spin glass in a random field,
+ *
+ *     H = - sum_<ij> J_ij s_i.s_j - sum_i H_i.s_i            (Eq. 1; each bond once)
+ *
+ * for D disorder samples x O replicas x T temperatures at once, with checkerboard
+ * over-relaxation (Eq. 3) and heat-bath (Eq. 2) sweeps, parallel-tempering swaps (Eq. 4) and the
+ * E / m / q^{mu nu}(k) reductions (Eqs. 5, 6).  DESIGN.md §3 fixes every arithmetic detail.
+ *
+ * Conventions
+ *   - Every pointer named *_dev is DEVICE memory owned by the caller (e.g. a torch tensor); pointers
+ *     named *_host are host memory.  The library never allocates or frees device memory: the caller
+ *     provides `dev_state` / `dev_scratch` of the sizes hsg_query_bytes() returns and keeps them alive
+ *     until hsg_destroy().  The layout inside them is private.
+ *   - Every call only ENQUEUES work on the CUDA stream given to hsg_create() (a cudaStream_t passed
+ *     as void*; NULL = the legacy default stream) and returns without synchronising; outputs are valid
+ *     once the caller has synchronised that stream.  The device current at hsg_create() must be
+ *     current at every later call.
+ *   - Site index i = x + L*(y + L*z), x fastest.  N = L^3.
+ *     J_dev[d][dir][i]: coupling of the bond from site i to site i+e_dir (dir 0,1,2 = x,y,z), periodic.
+ *     H_dev[d][c][i]  : component c of the field at site i.
+ *     S_dev[d][o][t][c][i]: component c of spin i of (sample d, replica o, TEMPERATURE index t).
+ *     All user-visible arrays are indexed by temperature index (0 = lowest T), never by the internal
+ *     memory slot a configuration sits in.
+ *   - P = O(O-1)/2 replica pairs in the order (0,1),(0,2),...,(1,2),...
+ *   - Return value: HSG_OK (0) or a negative error code; no exceptions, no exit().  Text of the last
+ *     error: hsg_last_error().  A context is not thread-safe; distinct contexts are independent.
+ *   - Determinism: the same descriptor, disorder, start spins and call sequence give bit-identical
+ *     results on every run, whatever kernel variant or grid is used (checkerboard independence,
+ *     PAPER.md:119, plus the counter-based random stream of DESIGN.md §3.5).
+ */
+#ifndef HSG_H_
+#define HSG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  HSG_OK = 0,
+  HSG_EINVAL = -1,       /* null pointer, odd or too small L, non-ascending temperatures, size mismatch */
+  HSG_ESTATE = -2,       /* e.g. sweep before disorder or spins were set */
+  HSG_EUNSUPPORTED = -3, /* lattice size / option not supported by the selected kernel */
+  HSG_ECUDA = -4         /* CUDA launch or runtime error; see hsg_last_error() */
+};
+
+/* kernel selection for hsg_sweep (hsg_set_option(HSG_OPT_SWEEP_KERNEL, ...)) */
+enum {
+  HSG_KERNEL_AUTO = 0,     /* fastest kernel that supports L */
+  HSG_KERNEL_GENERIC = 1,  /* one launch per colour, neighbours straight from global memory; any even L */
+  HSG_KERNEL_ZMARCH = 2    /* one launch per hsg_sweep call: both colours of every sweep fused in a z-marching pass */
+};
+enum {
+  HSG_OPT_SWEEP_KERNEL = 1
+};
+
+typedef struct hsg_ctx hsg_ctx; /* opaque, host side */
+
+typedef struct {
+  int32_t L;             /* lattice edge, even, >= 2 */
+  int32_t n_samples;     /* D >= 1 disorder samples held by this context */
+  int32_t n_replicas;    /* O >= 1 (overlaps need >= 2) */
+  int32_t n_temps;       /* T >= 1 */
+  const float* temps_host; /* T temperatures, strictly ascending, > 0; copied at create.
+                              beta_t = (float)(1.0/(double)temps[t]) */
+  uint64_t seed;         /* Philox key */
+  uint64_t sample_offset;/* global id of local sample 0: random streams are keyed by the global id
+                            sample_offset+d, so a job sharded by sample over several GPUs
+                            reproduces the single-GPU run */
+  uint32_t flags;        /* reserved, must be 0 */
+} hsg_desc;
+
+/* Sizes of the two caller-owned device buffers for this descriptor. */
+int hsg_query_bytes(const hsg_desc* desc, size_t* state_bytes, size_t* scratch_bytes);
+
+/* Create a context over caller-owned device buffers (256-byte aligned).  Enqueues initialisation of the
+ * permutation (configuration t holds temperature t) on `cuda_stream`. */
+int hsg_create(const hsg_desc* desc, void* dev_state, size_t state_bytes, void* dev_scratch,
+               size_t scratch_bytes, void* cuda_stream, hsg_ctx** out);
+
+/* Frees the host-side context only. */
+int hsg_destroy(hsg_ctx* ctx);
+
+/* Quenched disorder.  J_dev [D][3][N]; H_dev [D][3][N] or NULL for zero field.  The
+ * arrays are re-packed into the private layout; the caller may free them after synchronising. */
+int hsg_set_disorder(hsg_ctx* ctx, const float* J_dev, const float* H_dev);
+
+/* Start configuration: uniform on the sphere from the INIT domain of the random stream
+ * (DESIGN.md §3.5), for the temperature index each configuration currently holds. */
+int hsg_init_spins(hsg_ctx* ctx);
+
+/* Copy spins in / out, S_dev [D][O][T][3][N] fp32 by temperature index. */
+int hsg_set_spins(hsg_ctx* ctx, const float* S_dev);
+int hsg_get_spins(hsg_ctx* ctx, float* S_dev);
+
+/* n_or over-relaxation sweeps, THEN n_hb heat-bath sweeps of every system.
+ * One sweep = all even sites ((x+y+z)%2 == 0), then all odd sites.
+ * OR:  s' = 2 (s.h)/(h.h) h - s,  h = H_i + sum_j J_ij s_j                  (Eq. 3)
+ * HB:  s' ~ exp(beta h.s) from two uniforms of the Philox stream keyed by
+ *      (seed, sample, replica, temperature index, site, heat-bath sweep counter) (Eq. 2)
+ * The heat-bath sweep counter advances by one per HB sweep. */
+int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb);
+
+/* Total energy (Eq. 1) of every system, fp64, E_dev [D][O][T] by temperature index. */
+int hsg_energy(hsg_ctx* ctx, double* E_dev);
+
+/* One parallel-tempering pass (Eq. 4): for each (sample, replica), pairs (t, t+1) for
+ * t = 0..T-2 in this order, swap accepted with probability min[1, exp(dbeta*dE)],
+ * dE = E_{t+1}-E_t, dbeta = beta_{t+1}-beta_t, energies recomputed from the spins in fp64.
+ * accepted_dev [D][O][T-1] int32 (1 = swapped) or NULL.  The PT counter advances by one per call. */
+int hsg_pt_swap(hsg_ctx* ctx, int32_t* accepted_dev);
+
+/* Measurements, all fp64, any pointer may be NULL:
+ *   E_dev  [D][O][T]            total energy
+ *   M_dev  [D][O][T][3]         m = (1/N) sum_i s_i
+ *   q0_dev [D][P][T][3][3]      q^{mu nu}(0)      = (1/N) sum_i s_i^{mu(a)} s_i^{nu(b)}         (Eq. 5)
+ *   qk_dev [D][P][T][3][3][2]   q^{mu nu}(k_min)  = (1/N) sum_i s_i^{mu(a)} s_i^{nu(b)} e^{+i k x_i},
+ *                               k_min = (2 pi/L)(1,0,0), last index (re, im)        (Eq. 6)
+ * for replica pairs a<b holding the same temperature. */
+int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, double* qk_dev);
+
+/* Checkpoint: slot_of_temp_dev [D][O][T] int32 = configuration slot (0..T-1 within its (d,o) group, in
+ * hsg_init order) that holds temperature t; counters_host = {heat-bath sweep counter, PT counter}.
+ * hsg_get_state synchronises nothing: slot_of_temp_dev is written on the stream. */
+int hsg_get_state(hsg_ctx* ctx, int32_t* slot_of_temp_dev, uint64_t counters_host[2]);
+int hsg_set_state(hsg_ctx* ctx, const int32_t* slot_of_temp_dev, const uint64_t counters_host[2]);
+
+/* Tuning / test hooks (HSG_OPT_*).  Results never depend on them. */
+int hsg_set_option(hsg_ctx* ctx, int option, int value);
+
+/* Number of kernel launches enqueued by this context so far (for bench.py's gpu_launches). */
+uint64_t hsg_launch_count(const hsg_ctx* ctx);
+
+/* Name of the sweep kernel the last hsg_sweep used ("generic", "zmarch"; "none" before the first sweep). */
+const char* hsg_last_sweep_kernel(const hsg_ctx* ctx);
+
+const char* hsg_last_error(const hsg_ctx* ctx);
+const char* hsg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HSG_H_ */

@@ -1,0 +1,339 @@
+// hsg_api.cu — the C ABI of include/hsg.h: context bookkeeping and kernel launches.
+// All device work is enqueued on the stream given at hsg_create(); nothing here synchronises.
+#include "../../include/hsg.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "hsg_kernels.cuh"
+#include "hsg_zmarch.cuh"
+
+using namespace hsg;
+
+namespace {
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+// carve-up of the caller's two buffers (offsets in bytes)
+struct StateLayout {
+  size_t spins, jh, slot_of_temp, temp_of_slot, beta, cs_table, e_slot, m_slot, total;
+};
+struct ScratchLayout {
+  size_t e_partial, q_partial, total;
+};
+
+StateLayout state_layout(const Geom& g) {
+  StateLayout s{};
+  size_t o = 0;
+  s.spins = o;        o = align_up(o + sizeof(float) * 3 * (size_t)g.N * g.R);
+  s.jh = o;           o = align_up(o + sizeof(float) * 6 * (size_t)g.N * g.D);
+  s.slot_of_temp = o; o = align_up(o + sizeof(int32_t) * g.R);
+  s.temp_of_slot = o; o = align_up(o + sizeof(int32_t) * g.R);
+  s.beta = o;         o = align_up(o + sizeof(float) * g.T);
+  s.cs_table = o;     o = align_up(o + sizeof(double) * 2 * g.L);
+  s.e_slot = o;       o = align_up(o + sizeof(double) * g.R);
+  s.m_slot = o;       o = align_up(o + sizeof(double) * 3 * g.R);
+  s.total = o;
+  return s;
+}
+ScratchLayout scratch_layout(const Geom& g) {
+  ScratchLayout s{};
+  const size_t P = (size_t)g.O * (g.O - 1) / 2;
+  size_t o = 0;
+  s.e_partial = o; o = align_up(o + sizeof(double) * 4 * (size_t)g.R * g.L);
+  s.q_partial = o; o = align_up(o + sizeof(double) * 27 * (size_t)g.D * P * g.T * g.L);
+  s.total = o;
+  return s;
+}
+
+int check_desc(const hsg_desc* d) {
+  if (!d || !d->temps_host) return HSG_EINVAL;
+  if (d->L < 2 || (d->L & 1) || d->n_samples < 1 || d->n_replicas < 1 || d->n_temps < 1) return HSG_EINVAL;
+  if (d->flags != 0) return HSG_EINVAL;
+  for (int t = 0; t < d->n_temps; ++t) {
+    if (!(d->temps_host[t] > 0.0f) || !std::isfinite(d->temps_host[t])) return HSG_EINVAL;
+    if (t > 0 && !(d->temps_host[t] > d->temps_host[t - 1])) return HSG_EINVAL;
+  }
+  const double n = (double)d->L * d->L * d->L;
+  if (n > 2147483647.0) return HSG_EINVAL;                                   // site index is the 32-bit Philox word c0
+  if ((double)d->n_samples * d->n_replicas * d->n_temps > 1.0e9) return HSG_EINVAL;
+  return HSG_OK;
+}
+
+Geom make_geom(const hsg_desc* d) {
+  Geom g{};
+  g.L = d->L; g.Lh = d->L / 2;
+  g.D = d->n_samples; g.O = d->n_replicas; g.T = d->n_temps;
+  g.R = g.D * g.O * g.T;
+  g.N = (long long)d->L * d->L * d->L;
+  g.sample_offset = d->sample_offset;
+  return g;
+}
+
+inline unsigned blocks_for(long long n) { return (unsigned)((n + kThreads - 1) / kThreads); }
+
+}  // namespace
+
+struct hsg_ctx {
+  Geom g;
+  PhiloxKey key;
+  cudaStream_t stream;
+  // device pointers into the caller's buffers
+  float* spins; float* jh; int32_t* slot_of_temp; int32_t* temp_of_slot; float* beta; double* cs_table;
+  double* e_slot; double* m_slot; double* e_partial; double* q_partial;
+  unsigned long long k_hb, k_pt;
+  bool have_disorder, have_spins;
+  int sweep_kernel_opt;
+  const char* last_kernel;
+  unsigned long long launches;
+  std::string err;
+};
+
+#define HSG_FAIL(ctx, code, msg) do { (ctx)->err = (msg); return (code); } while (0)
+#define HSG_CUDA(ctx, expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { \
+  (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(e_); return HSG_ECUDA; } } while (0)
+#define HSG_LAUNCHED(ctx) do { ++(ctx)->launches; cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) { \
+  (ctx)->err = std::string("kernel launch: ") + cudaGetErrorString(e_); return HSG_ECUDA; } } while (0)
+
+extern "C" {
+
+const char* hsg_version(void) { return "hsg 0.1 (sm_100a)"; }
+
+int hsg_query_bytes(const hsg_desc* desc, size_t* state_bytes, size_t* scratch_bytes) {
+  const int rc = check_desc(desc);
+  if (rc != HSG_OK) return rc;
+  const Geom g = make_geom(desc);
+  if (state_bytes) *state_bytes = state_layout(g).total;
+  if (scratch_bytes) *scratch_bytes = scratch_layout(g).total;
+  return HSG_OK;
+}
+
+int hsg_create(const hsg_desc* desc, void* dev_state, size_t state_bytes, void* dev_scratch, size_t scratch_bytes,
+               void* cuda_stream, hsg_ctx** out) {
+  if (!out) return HSG_EINVAL;
+  *out = nullptr;
+  const int rc = check_desc(desc);
+  if (rc != HSG_OK) return rc;
+  const Geom g = make_geom(desc);
+  const StateLayout sl = state_layout(g);
+  const ScratchLayout cl = scratch_layout(g);
+  if (!dev_state || !dev_scratch || state_bytes < sl.total || scratch_bytes < cl.total) return HSG_EINVAL;
+  if (((uintptr_t)dev_state % kAlign) || ((uintptr_t)dev_scratch % kAlign)) return HSG_EINVAL;
+  hsg_ctx* c = new (std::nothrow) hsg_ctx();
+  if (!c) return HSG_EINVAL;
+  c->g = g;
+  c->key.k0 = (uint32_t)(desc->seed & 0xFFFFFFFFull);
+  c->key.k1 = (uint32_t)(desc->seed >> 32);
+  c->stream = (cudaStream_t)cuda_stream;
+  char* s = (char*)dev_state; char* w = (char*)dev_scratch;
+  c->spins = (float*)(s + sl.spins); c->jh = (float*)(s + sl.jh);
+  c->slot_of_temp = (int32_t*)(s + sl.slot_of_temp); c->temp_of_slot = (int32_t*)(s + sl.temp_of_slot);
+  c->beta = (float*)(s + sl.beta); c->cs_table = (double*)(s + sl.cs_table);
+  c->e_slot = (double*)(s + sl.e_slot); c->m_slot = (double*)(s + sl.m_slot);
+  c->e_partial = (double*)(w + cl.e_partial); c->q_partial = (double*)(w + cl.q_partial);
+  c->k_hb = 0; c->k_pt = 0; c->have_disorder = false; c->have_spins = false;
+  c->sweep_kernel_opt = HSG_KERNEL_AUTO; c->last_kernel = "none"; c->launches = 0;
+
+  // small host-computed tables: beta_t = (float)(1.0/(double)T_t); cos/sin(2 pi x / L) in fp64
+  std::vector<float> beta(g.T);
+  for (int t = 0; t < g.T; ++t) beta[t] = (float)(1.0 / (double)desc->temps_host[t]);
+  std::vector<double> cs(2 * (size_t)g.L);
+  const double two_pi = 6.283185307179586476925286766559;
+  for (int x = 0; x < g.L; ++x) {
+    const double ph = two_pi * (double)x / (double)g.L;
+    cs[2 * x] = std::cos(ph); cs[2 * x + 1] = std::sin(ph);
+  }
+  // pageable host memory: cudaMemcpyAsync stages it before returning, so the vectors may go out of scope
+  cudaError_t e = cudaMemcpyAsync(c->beta, beta.data(), sizeof(float) * g.T, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(c->cs_table, cs.data(), sizeof(double) * cs.size(), cudaMemcpyHostToDevice, c->stream);
+  if (e != cudaSuccess) { delete c; return HSG_ECUDA; }
+  init_perm_kernel<<<blocks_for(g.R), kThreads, 0, c->stream>>>(g, c->slot_of_temp, c->temp_of_slot);
+  ++c->launches;
+  if (cudaGetLastError() != cudaSuccess) { delete c; return HSG_ECUDA; }
+  *out = c;
+  return HSG_OK;
+}
+
+int hsg_destroy(hsg_ctx* ctx) {
+  if (!ctx) return HSG_EINVAL;
+  delete ctx;
+  return HSG_OK;
+}
+
+const char* hsg_last_error(const hsg_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+uint64_t hsg_launch_count(const hsg_ctx* ctx) { return ctx ? ctx->launches : 0; }
+const char* hsg_last_sweep_kernel(const hsg_ctx* ctx) { return ctx ? ctx->last_kernel : "none"; }
+
+int hsg_set_option(hsg_ctx* ctx, int option, int value) {
+  if (!ctx) return HSG_EINVAL;
+  if (option == HSG_OPT_SWEEP_KERNEL) {
+    if (value < HSG_KERNEL_AUTO || value > HSG_KERNEL_ZMARCH) HSG_FAIL(ctx, HSG_EINVAL, "unknown sweep kernel");
+    if (value == HSG_KERNEL_ZMARCH && !zmarch_supported(ctx->g)) HSG_FAIL(ctx, HSG_EUNSUPPORTED, "zmarch kernel does not support this geometry");
+    ctx->sweep_kernel_opt = value;
+    return HSG_OK;
+  }
+  HSG_FAIL(ctx, HSG_EINVAL, "unknown option");
+}
+
+int hsg_set_disorder(hsg_ctx* ctx, const float* J_dev, const float* H_dev) {
+  if (!ctx) return HSG_EINVAL;
+  if (!J_dev) HSG_FAIL(ctx, HSG_EINVAL, "J_dev is null");
+  pack_disorder_kernel<<<blocks_for((long long)ctx->g.D * ctx->g.N), kThreads, 0, ctx->stream>>>(ctx->g, J_dev, H_dev, ctx->jh);
+  HSG_LAUNCHED(ctx);
+  ctx->have_disorder = true;
+  return HSG_OK;
+}
+
+int hsg_init_spins(hsg_ctx* ctx) {
+  if (!ctx) return HSG_EINVAL;
+  init_spins_kernel<<<blocks_for((long long)ctx->g.R * ctx->g.N), kThreads, 0, ctx->stream>>>(ctx->g, ctx->key, ctx->temp_of_slot, ctx->spins);
+  HSG_LAUNCHED(ctx);
+  ctx->have_spins = true;
+  return HSG_OK;
+}
+
+int hsg_set_spins(hsg_ctx* ctx, const float* S_dev) {
+  if (!ctx) return HSG_EINVAL;
+  if (!S_dev) HSG_FAIL(ctx, HSG_EINVAL, "S_dev is null");
+  convert_spins_kernel<true><<<blocks_for((long long)ctx->g.R * ctx->g.N), kThreads, 0, ctx->stream>>>(
+      ctx->g, ctx->slot_of_temp, ctx->spins, const_cast<float*>(S_dev));
+  HSG_LAUNCHED(ctx);
+  ctx->have_spins = true;
+  return HSG_OK;
+}
+
+int hsg_get_spins(hsg_ctx* ctx, float* S_dev) {
+  if (!ctx) return HSG_EINVAL;
+  if (!S_dev) HSG_FAIL(ctx, HSG_EINVAL, "S_dev is null");
+  if (!ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "spins not set");
+  convert_spins_kernel<false><<<blocks_for((long long)ctx->g.R * ctx->g.N), kThreads, 0, ctx->stream>>>(
+      ctx->g, ctx->slot_of_temp, ctx->spins, S_dev);
+  HSG_LAUNCHED(ctx);
+  return HSG_OK;
+}
+
+// ------------------------------------------------------------------ sweeps
+static int launch_generic_sweep(hsg_ctx* ctx, bool hb) {
+  const Geom& g = ctx->g;
+  SweepArgs a{g, ctx->spins, ctx->jh, ctx->temp_of_slot, ctx->beta, ctx->key, ctx->k_hb};
+  const int V = (g.Lh % 4 == 0) ? 4 : (g.Lh % 2 == 0) ? 2 : 1;
+  const long long n = (long long)g.R * g.L * g.L * (g.Lh / V);
+  for (int colour = 0; colour < 2; ++colour) {
+    const unsigned nb = blocks_for(n);
+    if (V == 4) { if (hb) sweep_generic_kernel<4, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<4, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
+    else if (V == 2) { if (hb) sweep_generic_kernel<2, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<2, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
+    else { if (hb) sweep_generic_kernel<1, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<1, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
+    HSG_LAUNCHED(ctx);
+  }
+  return HSG_OK;
+}
+
+int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
+  if (!ctx) return HSG_EINVAL;
+  if (n_or < 0 || n_hb < 0) HSG_FAIL(ctx, HSG_EINVAL, "negative sweep count");
+  if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_sweep before disorder and spins were set");
+  if (n_or + n_hb == 0) return HSG_OK;
+  int kernel = ctx->sweep_kernel_opt;
+  if (kernel == HSG_KERNEL_AUTO) kernel = zmarch_supported(ctx->g) ? HSG_KERNEL_ZMARCH : HSG_KERNEL_GENERIC;
+  if (kernel == HSG_KERNEL_ZMARCH) {
+    ZmarchArgs a{ctx->g, ctx->spins, ctx->jh, ctx->temp_of_slot, ctx->beta, ctx->key, ctx->k_hb, n_or, n_hb};
+    int n_launch = 0;
+    const cudaError_t e = zmarch_launch(a, ctx->stream, &n_launch);
+    ctx->launches += (unsigned long long)n_launch;
+    if (e != cudaSuccess) { ctx->err = std::string("zmarch launch: ") + cudaGetErrorString(e); return HSG_ECUDA; }
+    ctx->k_hb += (unsigned long long)n_hb;
+    ctx->last_kernel = "zmarch";
+    return HSG_OK;
+  }
+  for (int s = 0; s < n_or; ++s) { const int rc = launch_generic_sweep(ctx, false); if (rc != HSG_OK) return rc; }
+  for (int s = 0; s < n_hb; ++s) {
+    const int rc = launch_generic_sweep(ctx, true);
+    if (rc != HSG_OK) return rc;
+    ++ctx->k_hb;
+  }
+  ctx->last_kernel = "generic";
+  return HSG_OK;
+}
+
+// ------------------------------------------------------------------ energy, parallel tempering, measurements
+static int enqueue_energy_mag(hsg_ctx* ctx) {
+  const Geom& g = ctx->g;
+  energy_mag_kernel<<<(unsigned)((long long)g.R * g.L), kThreads, 0, ctx->stream>>>(g, ctx->spins, ctx->jh, ctx->e_partial);
+  HSG_LAUNCHED(ctx);
+  finalize_energy_kernel<<<blocks_for((long long)g.R * 4), kThreads, 0, ctx->stream>>>(g, ctx->e_partial, ctx->e_slot, ctx->m_slot);
+  HSG_LAUNCHED(ctx);
+  return HSG_OK;
+}
+
+int hsg_energy(hsg_ctx* ctx, double* E_dev) {
+  if (!ctx) return HSG_EINVAL;
+  if (!E_dev) HSG_FAIL(ctx, HSG_EINVAL, "E_dev is null");
+  if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_energy before disorder and spins were set");
+  const int rc = enqueue_energy_mag(ctx);
+  if (rc != HSG_OK) return rc;
+  gather_by_temp_kernel<<<blocks_for(ctx->g.R), kThreads, 0, ctx->stream>>>(ctx->g, 1, ctx->slot_of_temp, ctx->e_slot, E_dev);
+  HSG_LAUNCHED(ctx);
+  return HSG_OK;
+}
+
+int hsg_pt_swap(hsg_ctx* ctx, int32_t* accepted_dev) {
+  if (!ctx) return HSG_EINVAL;
+  if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_pt_swap before disorder and spins were set");
+  const int rc = enqueue_energy_mag(ctx);
+  if (rc != HSG_OK) return rc;
+  pt_swap_kernel<<<blocks_for((long long)ctx->g.D * ctx->g.O), kThreads, 0, ctx->stream>>>(
+      ctx->g, ctx->key, ctx->k_pt, ctx->beta, ctx->e_slot, ctx->slot_of_temp, ctx->temp_of_slot, accepted_dev);
+  HSG_LAUNCHED(ctx);
+  ++ctx->k_pt;
+  return HSG_OK;
+}
+
+int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, double* qk_dev) {
+  if (!ctx) return HSG_EINVAL;
+  if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_measure before disorder and spins were set");
+  const Geom& g = ctx->g;
+  if (E_dev || M_dev) {
+    const int rc = enqueue_energy_mag(ctx);
+    if (rc != HSG_OK) return rc;
+    if (E_dev) { gather_by_temp_kernel<<<blocks_for(g.R), kThreads, 0, ctx->stream>>>(g, 1, ctx->slot_of_temp, ctx->e_slot, E_dev); HSG_LAUNCHED(ctx); }
+    if (M_dev) { gather_by_temp_kernel<<<blocks_for((long long)g.R * 3), kThreads, 0, ctx->stream>>>(g, 3, ctx->slot_of_temp, ctx->m_slot, M_dev); HSG_LAUNCHED(ctx); }
+  }
+  const int P = g.O * (g.O - 1) / 2;
+  if ((q0_dev || qk_dev) && P > 0) {
+    const long long n_sys = (long long)g.D * P * g.T;
+    overlap_kernel<<<(unsigned)(n_sys * g.L), kThreads, 0, ctx->stream>>>(g, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+    HSG_LAUNCHED(ctx);
+    finalize_overlap_kernel<<<blocks_for(n_sys * 9), kThreads, 0, ctx->stream>>>(g, (int)n_sys, ctx->q_partial, q0_dev, qk_dev);
+    HSG_LAUNCHED(ctx);
+  }
+  return HSG_OK;
+}
+
+// ------------------------------------------------------------------ checkpoint
+int hsg_get_state(hsg_ctx* ctx, int32_t* slot_of_temp_dev, uint64_t counters_host[2]) {
+  if (!ctx) return HSG_EINVAL;
+  if (slot_of_temp_dev)
+    HSG_CUDA(ctx, cudaMemcpyAsync(slot_of_temp_dev, ctx->slot_of_temp, sizeof(int32_t) * ctx->g.R, cudaMemcpyDeviceToDevice, ctx->stream));
+  if (counters_host) { counters_host[0] = ctx->k_hb; counters_host[1] = ctx->k_pt; }
+  return HSG_OK;
+}
+
+int hsg_set_state(hsg_ctx* ctx, const int32_t* slot_of_temp_dev, const uint64_t counters_host[2]) {
+  if (!ctx) return HSG_EINVAL;
+  if (slot_of_temp_dev) {
+    // NOTE: the caller must pass a valid permutation per (sample, replica); spins stay in their slots.
+    set_perm_kernel<<<blocks_for(ctx->g.R), kThreads, 0, ctx->stream>>>(ctx->g, slot_of_temp_dev, ctx->slot_of_temp, ctx->temp_of_slot);
+    HSG_LAUNCHED(ctx);
+  }
+  if (counters_host) { ctx->k_hb = counters_host[0]; ctx->k_pt = counters_host[1]; }
+  return HSG_OK;
+}
+
+}  // extern "C"

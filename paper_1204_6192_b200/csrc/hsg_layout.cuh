@@ -1,0 +1,39 @@
+// hsg_layout.cuh — private HBM layout of the engine.
+//
+// Checkerboard-compacted, plane-major SoA.  A site (x,y,z) has colour c = (x+y+z)&1 and compact
+// x-index j = x>>1, i.e. x = 2j + ((y+z+c)&1); Lh = L/2.
+//   spins of one configuration slot : S[z][c][mu][y][j]    fp32, 3N floats   (mu = spin component)
+//   disorder of one sample          : JH[z][c][k][y][j]    fp32, 6N floats   k=0,1,2: J of the bond
+//                                     from this site to +x,+y,+z ; k=3,4,5: H_x,H_y,H_z
+// so that (i) all sites a colour update touches are unit-stride in j (128-bit vector loads, one
+// colour never interleaved with the other), (ii) the four y/z neighbours of compact site j sit at the
+// SAME j in the other colour's rows, the x neighbours at j and j-1 (or j+1), and (iii) one z-plane of
+// one colour is a single contiguous block (3*L*Lh floats) that a bulk async copy can move.
+#pragma once
+#include <cstdint>
+
+namespace hsg {
+
+struct Geom {
+  int L, Lh;          // lattice edge, L/2
+  int D, O, T;        // samples, replicas, temperatures
+  int R;              // D*O*T systems
+  long long N;        // L^3
+  unsigned long long sample_offset;
+};
+
+__host__ __device__ __forceinline__ long long row_elems(const Geom& g) { return g.Lh; }
+__host__ __device__ __forceinline__ long long comp_elems(const Geom& g) { return (long long)g.L * g.Lh; }   // one [y][j] array
+__host__ __device__ __forceinline__ long long spin_halfplane(const Geom& g) { return 3 * comp_elems(g); }
+__host__ __device__ __forceinline__ long long spin_plane(const Geom& g) { return 6 * comp_elems(g); }
+__host__ __device__ __forceinline__ long long jh_halfplane(const Geom& g) { return 6 * comp_elems(g); }
+__host__ __device__ __forceinline__ long long jh_plane(const Geom& g) { return 12 * comp_elems(g); }
+
+__host__ __device__ __forceinline__ long long spin_index(const Geom& g, int z, int c, int mu, int y, int j) {
+  return (((long long)(z * 2 + c) * 3 + mu) * g.L + y) * g.Lh + j;
+}
+__host__ __device__ __forceinline__ long long jh_index(const Geom& g, int z, int c, int k, int y, int j) {
+  return (((long long)(z * 2 + c) * 6 + k) * g.L + y) * g.Lh + j;
+}
+
+}  // namespace hsg
