@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py — headline measurement of the hsg hot path (BASELINE.json metric: ns per spin update, OR+HB mix).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+One "step" is one pass of the whole hot path over every system of the workload:
+hsg_sweep(n_or, n_hb) + hsg_pt_swap (energies + swaps) + hsg_measure (E, m, q(0), q(k_min)).
+`value` = step time / ((n_or+n_hb) * R * N) in ns, state resident in HBM (1.6 GB for c4, far larger than L2).
+`e2e`   = the same metric over one "execution round" driven through the C ABI from HOST
+          buffers: J, H and the start spins are copied from pinned host memory, K steps run with the
+          observables of every step read back to the host, and the final spins are read back — all inside
+          the timed region; bytes per step = round bytes / K.
+`roofline` is for the sweep kernel (the dominant one): algorithmic bytes / CUDA-event time.
+`cpu_baseline` = the oracle (oracle/, as it stands) timed on the host cores on a bounded sample.
+Rank r of an N-GPU run owns its own D samples (sample_offset = r*D): weak scaling, no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import hsg_inputs  # noqa: E402
+
+METRIC = "ns per spin update (OR+HB mix)"
+UNIT = "ns/update"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _traffic(workload, kernel):
+    """dram bytes per sweep-kernel launch from the committed ncu capture (profiles/traffic.json), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get(f"{workload}:{kernel}")
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _dist():
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    return rank, world, int(os.environ.get("LOCAL_RANK", 0))
+
+
+# ------------------------------------------------------------------------------------------------ oracle arms
+def run_oracle(cfg, temps, steps, warmup, n_systems_cap=64):
+    """Time the oracle as it stands on a bounded sample of the workload: the first sample's systems
+    (at most n_systems_cap of them), `steps` full steps after `warmup`.  Returns (ns/update, cores, text)."""
+    import oracle
+    cores = os.cpu_count() or 1
+    O = cfg["n_replicas"]
+    T = len(temps)
+    while O * T > n_systems_cap and T > 2:
+        T //= 2
+    tsub = temps[:: len(temps) // T][:T]
+    L = cfg["L"]
+    J = hsg_inputs.couplings(L, 1, cfg["seed"])
+    H = hsg_inputs.gaussian_field(L, 1, cfg["h_r"], cfg["seed"]) if cfg["h_r"] > 0 else None
+    sim = oracle.Oracle(L, 1, O, tsub, cfg["seed"], precision=32, n_threads=cores)
+    sim.set_disorder(J, H); sim.init_spins()
+    def step():
+        sim.sweep(cfg["n_or"], cfg["n_hb"]); sim.pt_swap(); sim.measure()
+    for _ in range(warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        step()
+    dt = time.perf_counter() - t0
+    updates = (cfg["n_or"] + cfg["n_hb"]) * O * T * L ** 3 * steps
+    text = (f"{steps} steps ({cfg['n_or']} OR + {cfg['n_hb']} HB + PT + measure) of 1 sample x {O} replicas x {T} temperatures, "
+            f"L={L}, fp32 oracle, {cores} threads over systems")
+    return dt / updates * 1e9, cores, text, dt / steps * 1e3
+
+
+def main_reference(args, cfg, temps):
+    rank, world, _ = _dist()
+    if rank != 0:
+        return
+    ns, cores, text, ms = run_oracle(cfg, temps, max(1, args.steps), max(0, min(args.warmup, 1)))
+    line = {"impl": "reference", "metric": METRIC, "value": ns, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": {"workload": args.workload, "note": "oracle on host cores, bounded sample"},
+            "cpu_baseline": {"value": ns, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text},
+            "e2e": {"value": ns, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ GPU arm
+def main_ours(args, cfg, temps):
+    import torch
+    import paper_1204_6192_b200 as hsg
+
+    rank, world, local = _dist()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hsg hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    L, D, O, T = cfg["L"], cfg["n_samples"], cfg["n_replicas"], len(temps)
+    n_or, n_hb = cfg["n_or"], cfg["n_hb"]
+    N, R = L ** 3, D * O * T
+    off = rank * D                                     # weak scaling: every rank owns its own D samples
+    J = hsg_inputs.couplings(L, D, cfg["seed"], off)
+    H = hsg_inputs.gaussian_field(L, D, cfg["h_r"], cfg["seed"], off) if cfg["h_r"] > 0 else None
+
+    eng = hsg.hsg_create(L, D, O, temps, cfg["seed"], sample_offset=off, kernel=args.kernel)
+    eng.set_disorder(J, H)
+    eng.init_spins()
+    f64, i32 = torch.float64, torch.int32
+    outs = (eng._new((D, O, T), f64), eng._new((D, O, T, 3), f64), eng._new((D, eng.P, T, 3, 3), f64), eng._new((D, eng.P, T, 3, 3, 2), f64))
+    acc = eng._new((D, O, max(T - 1, 0)), i32)
+    measure = not args.no_measure
+
+    def step():
+        eng.sweep(n_or, n_hb)
+        eng.pt_swap(out=acc)
+        if measure:
+            eng.measure(out=outs)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+    launches0 = eng.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 2)]
+    ev[0].record()
+    for k in range(args.steps):
+        ev[2 + 2 * k].record()
+        eng.sweep(n_or, n_hb)
+        ev[3 + 2 * k].record()
+        eng.pt_swap(out=acc)
+        if measure:
+            eng.measure(out=outs)
+    ev[1].record()
+    barrier()
+    launches = eng.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    total_ms = ev[0].elapsed_time(ev[1])
+    sweep_ms = sum(ev[2 + 2 * k].elapsed_time(ev[3 + 2 * k]) for k in range(args.steps))
+    if dist is not None:
+        t = torch.tensor([total_ms, sweep_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, sweep_ms = t.tolist()
+    kernel = eng.last_sweep_kernel()
+    sweep_launches_per_call = 1 if kernel == "zmarch" else 2 * (n_or + n_hb)
+
+    # ---- end-to-end round through the C ABI from host buffers (rank-local; max over ranks)
+    e2e = None
+    if not args.no_e2e:
+        S0 = eng.get_spins()
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        J_h, H_h = pin(J), (pin(H) if H is not None else None)
+        S_h = torch.empty(S0.shape, dtype=torch.float32).pin_memory(); S_h.copy_(S0); del S0
+        out_h = [torch.empty(o.shape, dtype=o.dtype).pin_memory() for o in outs] + [torch.empty(acc.shape, dtype=i32).pin_memory()]
+        S_back = torch.empty(S_h.shape, dtype=torch.float32).pin_memory()
+        S_dev = eng._new(S_h.shape, torch.float32)
+        J_dev = eng._new(J_h.shape, torch.float32); H_dev = eng._new(J_h.shape, torch.float32) if H_h is not None else None
+        def round_():
+            J_dev.copy_(J_h, non_blocking=True)
+            if H_dev is not None:
+                H_dev.copy_(H_h, non_blocking=True)
+            S_dev.copy_(S_h, non_blocking=True)
+            eng.set_disorder(J_dev, H_dev); eng.set_spins(S_dev)
+            for _ in range(args.steps):
+                eng.sweep(n_or, n_hb)
+                eng.pt_swap(out=acc)
+                eng.measure(out=outs)
+                for h, d in zip(out_h, list(outs) + [acc]):
+                    h.copy_(d, non_blocking=True)
+            eng.get_spins(out=S_dev)
+            S_back.copy_(S_dev, non_blocking=True)
+        round_()                                            # warm-up round
+        barrier()
+        t0 = time.perf_counter()
+        round_()
+        barrier()
+        e2e_s = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = t.item()
+        h2d = (J_h.numel() + (H_h.numel() if H_h is not None else 0) + S_h.numel()) * 4
+        d2h = S_back.numel() * 4 + args.steps * sum(h.numel() * h.element_size() for h in out_h)
+        e2e = {"value": e2e_s * 1e9 / ((n_or + n_hb) * R * N * args.steps), "unit": UNIT,
+               "h2d_bytes_per_step": h2d // args.steps, "d2h_bytes_per_step": d2h // args.steps,
+               "what": f"one round of {args.steps} steps: J,H,spins H2D from pinned host + steps with per-step observables D2H + spins D2H"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    updates_step = (n_or + n_hb) * R * N                       # per rank
+    ms_step = total_ms / args.steps
+    value = ms_step * 1e6 / updates_step / world               # whole job: all ranks' updates in that time
+    ns_sweeps = sweep_ms / args.steps * 1e6 / updates_step / world
+    # roofline of the sweep kernel: algorithmic bytes per update:
+    # every spin read and written once per sweep (24 B) + J,H once per sweep per sample (24 B / (O*T))
+    bytes_per_update = 24.0 + 24.0 / (O * T)
+    peak, peak_src = _peaks()
+    per_launch_updates = updates_step / sweep_launches_per_call
+    launch_ms = sweep_ms / args.steps / sweep_launches_per_call
+    achieved = bytes_per_update * per_launch_updates / (launch_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": _traffic(args.workload, kernel), "kernel": f"sweep ({kernel})", "peak_source": peak_src,
+                "bytes_per_update": bytes_per_update, "launch_ms": launch_ms, "sweep_share_of_step": sweep_ms / total_ms}
+
+    if args.cpu_steps > 0:
+        ns_cpu, cores, text, _ = run_oracle(cfg, temps, args.cpu_steps, 1)
+    else:
+        ns_cpu, cores, text = None, 0, "skipped (--cpu-steps 0)"
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": f"{args.workload}: L={L}, {D} samples x {O} replicas x {T} temperatures per GPU, "
+                                   f"{n_or} OR + {n_hb} HB + PT{' + measure' if measure else ''} per step",
+                       "L": L, "n_samples_per_gpu": D, "n_replicas": O, "n_temps": T, "n_or": n_or, "n_hb": n_hb,
+                       "parallelism": f"samples sharded over {world} GPU(s), no collective", "sweep_kernel": kernel,
+                       "l2": "state (spins) far larger than L2; no flush needed"},
+            "ns_per_update_sweeps_only": ns_sweeps, "roofline": roofline,
+            "cpu_baseline": {"value": ns_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text},
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "paper_context": {"gtx480_ns_per_update_1hb_100or": 0.29, "gtx480_1hb_10or": 0.45, "note": "PAPER.md Table 1, other hardware"}}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", choices=sorted(hsg_inputs.CONFIGS))
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "zmarch"])
+    ap.add_argument("--samples", type=int, default=None, help="override the number of disorder samples per GPU")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-measure", action="store_true")
+    ap.add_argument("--cpu-steps", type=int, default=3, help="oracle steps timed for cpu_baseline")
+    args = ap.parse_args()
+    cfg = dict(hsg_inputs.CONFIGS[args.workload])
+    if args.samples is not None:
+        cfg["n_samples"] = args.samples
+    if cfg["t_min"] == cfg["t_max"]:
+        temps = (cfg["t_min"] * (1.0 + 1e-6 * np.arange(cfg["n_temps"]))).astype(np.float32)
+    else:
+        temps = hsg_inputs.geometric_ladder(cfg["t_min"], cfg["t_max"], cfg["n_temps"])
+    if args.impl == "reference":
+        main_reference(args, cfg, temps)
+    else:
+        main_ours(args, cfg, temps)
+
+
+if __name__ == "__main__":
+    main()
