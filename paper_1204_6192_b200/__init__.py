@@ -26,7 +26,7 @@ KERNELS = {"auto": HSG_KERNEL_AUTO, "generic": HSG_KERNEL_GENERIC, "zmarch": HSG
 SYMBOLS = (
     "hsg_query_bytes", "hsg_create", "hsg_destroy", "hsg_set_disorder", "hsg_init_spins", "hsg_set_spins",
     "hsg_get_spins", "hsg_sweep", "hsg_energy", "hsg_pt_swap", "hsg_measure", "hsg_get_state", "hsg_set_state",
-    "hsg_set_option", "hsg_launch_count", "hsg_last_sweep_kernel", "hsg_last_error", "hsg_version",
+    "hsg_set_option", "hsg_launch_count", "hsg_last_sweep_kernel", "hsg_last_error", "hsg_version", "hsg_selftest_arith",
 )
 
 
@@ -70,12 +70,23 @@ def lib() -> C.CDLL:
         L.hsg_last_sweep_kernel.argtypes = [vp]; L.hsg_last_sweep_kernel.restype = C.c_char_p
         L.hsg_last_error.argtypes = [vp]; L.hsg_last_error.restype = C.c_char_p
         L.hsg_version.argtypes = []; L.hsg_version.restype = C.c_char_p
+        L.hsg_selftest_arith.argtypes = [vp, C.c_uint64, C.c_uint64, vp]
         _LIB = L
     return _LIB
 
 
 def hsg_version() -> str:
     return lib().hsg_version().decode()
+
+
+def hsg_selftest_arith(n, seed=1):
+    """(division mismatches, square-root mismatches) of the kernels' branch-free IEEE routines over n operand sets."""
+    import torch
+    counts = torch.zeros(2, dtype=torch.int64, device="cuda")
+    rc = lib().hsg_selftest_arith(C.c_void_p(torch.cuda.current_stream().cuda_stream), int(seed), int(n), counts.data_ptr())
+    if rc != HSG_OK:
+        raise HsgError(rc, "hsg_selftest_arith failed")
+    return tuple(int(x) for x in counts.cpu())
 
 
 def hsg_query_bytes(L, n_samples, n_replicas, temps, seed=0, sample_offset=0):

@@ -90,6 +90,7 @@ struct hsg_ctx {
   double* e_slot; double* m_slot; double* e_partial; double* q_partial;
   unsigned long long k_hb, k_pt;
   bool have_disorder, have_spins;
+  bool energy_valid;            // e_slot / m_slot hold the reduction of the current spins
   int sweep_kernel_opt;
   const char* last_kernel;
   unsigned long long launches;
@@ -138,7 +139,7 @@ int hsg_create(const hsg_desc* desc, void* dev_state, size_t state_bytes, void* 
   c->beta = (float*)(s + sl.beta); c->cs_table = (double*)(s + sl.cs_table);
   c->e_slot = (double*)(s + sl.e_slot); c->m_slot = (double*)(s + sl.m_slot);
   c->e_partial = (double*)(w + cl.e_partial); c->q_partial = (double*)(w + cl.q_partial);
-  c->k_hb = 0; c->k_pt = 0; c->have_disorder = false; c->have_spins = false;
+  c->k_hb = 0; c->k_pt = 0; c->have_disorder = false; c->have_spins = false; c->energy_valid = false;
   c->sweep_kernel_opt = HSG_KERNEL_AUTO; c->last_kernel = "none"; c->launches = 0;
 
   // small host-computed tables: beta_t = (float)(1.0/(double)T_t); cos/sin(2 pi x / L) in fp64
@@ -188,6 +189,7 @@ int hsg_set_disorder(hsg_ctx* ctx, const float* J_dev, const float* H_dev) {
   pack_disorder_kernel<<<blocks_for((long long)ctx->g.D * ctx->g.N), kThreads, 0, ctx->stream>>>(ctx->g, J_dev, H_dev, ctx->jh);
   HSG_LAUNCHED(ctx);
   ctx->have_disorder = true;
+  ctx->energy_valid = false;
   return HSG_OK;
 }
 
@@ -196,6 +198,7 @@ int hsg_init_spins(hsg_ctx* ctx) {
   init_spins_kernel<<<blocks_for((long long)ctx->g.R * ctx->g.N), kThreads, 0, ctx->stream>>>(ctx->g, ctx->key, ctx->temp_of_slot, ctx->spins);
   HSG_LAUNCHED(ctx);
   ctx->have_spins = true;
+  ctx->energy_valid = false;
   return HSG_OK;
 }
 
@@ -206,6 +209,7 @@ int hsg_set_spins(hsg_ctx* ctx, const float* S_dev) {
       ctx->g, ctx->slot_of_temp, ctx->spins, const_cast<float*>(S_dev));
   HSG_LAUNCHED(ctx);
   ctx->have_spins = true;
+  ctx->energy_valid = false;
   return HSG_OK;
 }
 
@@ -240,6 +244,7 @@ int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
   if (n_or < 0 || n_hb < 0) HSG_FAIL(ctx, HSG_EINVAL, "negative sweep count");
   if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_sweep before disorder and spins were set");
   if (n_or + n_hb == 0) return HSG_OK;
+  ctx->energy_valid = false;
   int kernel = ctx->sweep_kernel_opt;
   if (kernel == HSG_KERNEL_AUTO) kernel = zmarch_supported(ctx->g) ? HSG_KERNEL_ZMARCH : HSG_KERNEL_GENERIC;
   if (kernel == HSG_KERNEL_ZMARCH) {
@@ -263,12 +268,28 @@ int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
 }
 
 // ------------------------------------------------------------------ energy, parallel tempering, measurements
+// planes per block of the reduction kernels: about 4 vector items per thread, at most L chunks per system
+static int reduce_zb(const Geom& g, int V) {
+  const int ipp = 2 * g.L * (g.Lh / V);
+  int zb = (4 * kThreads + ipp - 1) / ipp;
+  if (zb < 1) zb = 1;
+  if (zb > g.L) zb = g.L;
+  return zb;
+}
+static int vec_width(const Geom& g) { return (g.Lh % 4 == 0) ? 4 : (g.Lh % 2 == 0) ? 2 : 1; }
+
 static int enqueue_energy_mag(hsg_ctx* ctx) {
   const Geom& g = ctx->g;
-  energy_mag_kernel<<<(unsigned)((long long)g.R * g.L), kThreads, 0, ctx->stream>>>(g, ctx->spins, ctx->jh, ctx->e_partial);
+  if (ctx->energy_valid) return HSG_OK;          // spins unchanged since the last reduction
+  const int V = vec_width(g), ZB = reduce_zb(g, V), n_chunks = (g.L + ZB - 1) / ZB;
+  const unsigned nb = (unsigned)((long long)g.R * n_chunks);
+  if (V == 4) energy_mag_kernel<4><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->jh, ctx->e_partial);
+  else if (V == 2) energy_mag_kernel<2><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->jh, ctx->e_partial);
+  else energy_mag_kernel<1><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->jh, ctx->e_partial);
   HSG_LAUNCHED(ctx);
-  finalize_energy_kernel<<<blocks_for((long long)g.R * 4), kThreads, 0, ctx->stream>>>(g, ctx->e_partial, ctx->e_slot, ctx->m_slot);
+  finalize_energy_kernel<<<blocks_for((long long)g.R * 4), kThreads, 0, ctx->stream>>>(g, n_chunks, ctx->e_partial, ctx->e_slot, ctx->m_slot);
   HSG_LAUNCHED(ctx);
+  ctx->energy_valid = true;
   return HSG_OK;
 }
 
@@ -308,12 +329,26 @@ int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, doub
   const int P = g.O * (g.O - 1) / 2;
   if ((q0_dev || qk_dev) && P > 0) {
     const long long n_sys = (long long)g.D * P * g.T;
-    overlap_kernel<<<(unsigned)(n_sys * g.L), kThreads, 0, ctx->stream>>>(g, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+    const int V = vec_width(g), ZB = reduce_zb(g, V), n_chunks = (g.L + ZB - 1) / ZB;
+    const unsigned nb = (unsigned)(n_sys * n_chunks);
+    if (V == 4) overlap_kernel<4><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+    else if (V == 2) overlap_kernel<2><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+    else overlap_kernel<1><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
     HSG_LAUNCHED(ctx);
-    finalize_overlap_kernel<<<blocks_for(n_sys * 9), kThreads, 0, ctx->stream>>>(g, (int)n_sys, ctx->q_partial, q0_dev, qk_dev);
+    finalize_overlap_kernel<<<blocks_for(n_sys * 9), kThreads, 0, ctx->stream>>>(g, (int)n_sys, n_chunks, ctx->q_partial, q0_dev, qk_dev);
     HSG_LAUNCHED(ctx);
   }
   return HSG_OK;
+}
+
+// ------------------------------------------------------------------ arithmetic self-test
+int hsg_selftest_arith(void* cuda_stream, uint64_t seed, uint64_t n, unsigned long long* counts_dev) {
+  if (!counts_dev) return HSG_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (cudaMemsetAsync(counts_dev, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return HSG_ECUDA;
+  PhiloxKey key{(uint32_t)seed, (uint32_t)(seed >> 32)};
+  selftest_arith_kernel<<<148 * 8, kThreads, 0, st>>>(key, n, counts_dev);
+  return cudaGetLastError() == cudaSuccess ? HSG_OK : HSG_ECUDA;
 }
 
 // ------------------------------------------------------------------ checkpoint

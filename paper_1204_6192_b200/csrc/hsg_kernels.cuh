@@ -237,49 +237,74 @@ __device__ __forceinline__ void block_reduce_store(double (&v)[NV], double* __re
 }
 
 // ------------------------------------------------------------------ energy (Eq. 1) and magnetisation per slot
-// One block per (slot, z-plane).  partial[slot][z][4] = { -E contribution, sum s_x, sum s_y, sum s_z }.
+// One block per (slot, chunk of ZB planes); each thread takes items of V compact sites of one colour
+// (vector loads: own spins, the +x, +y, +z neighbours in the other colour's arrays, J and H), i.e. every
+// bond once.  partial[slot][chunk][4] = { -E contribution, sum s_x, sum s_y, sum s_z }.
 // Every fp32*fp32 product is exact in fp64; sums are fp64.
-__global__ void __launch_bounds__(kThreads) energy_mag_kernel(Geom g, const float* __restrict__ spins, const float* __restrict__ jh,
+template <int V>
+__global__ void __launch_bounds__(kThreads) energy_mag_kernel(Geom g, int ZB, const float* __restrict__ spins, const float* __restrict__ jh,
                                                               double* __restrict__ partial) {
-  const int L = g.L, Lh = g.Lh;
-  const int slot = blockIdx.x / L, z = blockIdx.x % L;
-  const int zp = (z + 1 == L) ? 0 : z + 1;
+  const int L = g.L, Lh = g.Lh, qpr = Lh / V;
+  const int n_chunks = (L + ZB - 1) / ZB;
+  const int slot = blockIdx.x / n_chunks, chunk = blockIdx.x % n_chunks;
+  const int z0 = chunk * ZB, nz = min(ZB, L - z0);
   const float* S = spins + (long long)slot * 3 * g.N;
   const float* JH = jh + (long long)(slot / (g.O * g.T)) * 6 * g.N;
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
-  const int per_plane = 2 * L * Lh;
-  for (int idx = threadIdx.x; idx < per_plane; idx += kThreads) {
-    const int j = idx % Lh; int rem = idx / Lh;
-    const int y = rem % L; const int c = rem / L;
-    const int cc = 1 - c;
+  const int ipp = 2 * L * qpr;                      // items per plane
+  for (int it = threadIdx.x; it < nz * ipp; it += kThreads) {
+    const int q = it % qpr; int rem = it / qpr;
+    const int y = rem % L; rem /= L;
+    const int c = rem & 1; const int z = z0 + (rem >> 1);
+    const int cc = 1 - c, j0 = q * V;
     const int off = (y + z + c) & 1;
-    const int yp = (y + 1 == L) ? 0 : y + 1;
-    const int jxp = off ? ((j + 1 == Lh) ? 0 : j + 1) : j;
-    double s[3], dx = 0.0, dy = 0.0, dz = 0.0, hs = 0.0;
+    const int yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
+    const int je = (j0 + V == Lh) ? 0 : j0 + V;     // +x neighbour outside the vector (used when off = 1)
+    const Vec<V> Jx = ldv<V>(JH + jh_index(g, z, c, 0, y, j0));
+    const Vec<V> Jy = ldv<V>(JH + jh_index(g, z, c, 1, y, j0));
+    const Vec<V> Jz = ldv<V>(JH + jh_index(g, z, c, 2, y, j0));
+    double dx[V], dy[V], dz[V], hs[V];
+#pragma unroll
+    for (int e = 0; e < V; ++e) { dx[e] = 0.0; dy[e] = 0.0; dz[e] = 0.0; hs[e] = 0.0; }
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) {
-      s[mu] = (double)S[spin_index(g, z, c, mu, y, j)];
-      dx = fma(s[mu], (double)S[spin_index(g, z, cc, mu, y, jxp)], dx);
-      dy = fma(s[mu], (double)S[spin_index(g, z, cc, mu, yp, j)], dy);
-      dz = fma(s[mu], (double)S[spin_index(g, zp, cc, mu, y, j)], dz);
-      hs = fma((double)JH[jh_index(g, z, c, 3 + mu, y, j)], s[mu], hs);
-      acc[1 + mu] += s[mu];
+      const Vec<V> s = ldv<V>(S + spin_index(g, z, c, mu, y, j0));
+      const Vec<V> sx = ldv<V>(S + spin_index(g, z, cc, mu, y, j0));
+      const float se = off ? S[spin_index(g, z, cc, mu, y, je)] : 0.0f;
+      const Vec<V> sy = ldv<V>(S + spin_index(g, z, cc, mu, yp, j0));
+      const Vec<V> sz = ldv<V>(S + spin_index(g, zp, cc, mu, y, j0));
+      const Vec<V> Hm = ldv<V>(JH + jh_index(g, z, c, 3 + mu, y, j0));
+      double msum = 0.0;
+#pragma unroll
+      for (int e = 0; e < V; ++e) {
+        const double sd = (double)s.v[e];
+        const float xn = off ? (e + 1 < V ? sx.v[e + 1 < V ? e + 1 : 0] : se) : sx.v[e];
+        dx[e] = fma(sd, (double)xn, dx[e]);
+        dy[e] = fma(sd, (double)sy.v[e], dy[e]);
+        dz[e] = fma(sd, (double)sz.v[e], dz[e]);
+        hs[e] = fma((double)Hm.v[e], sd, hs[e]);
+        msum += sd;
+      }
+      acc[1 + mu] += msum;
     }
-    double e = (double)JH[jh_index(g, z, c, 0, y, j)] * dx;
-    e = fma((double)JH[jh_index(g, z, c, 1, y, j)], dy, e);
-    e = fma((double)JH[jh_index(g, z, c, 2, y, j)], dz, e);
-    acc[0] += e + hs;
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+      double en = (double)Jx.v[e] * dx[e];
+      en = fma((double)Jy.v[e], dy[e], en);
+      en = fma((double)Jz.v[e], dz[e], en);
+      acc[0] += en + hs[e];
+    }
   }
-  block_reduce_store<4>(acc, partial + ((long long)slot * L + z) * 4);
+  block_reduce_store<4>(acc, partial + (long long)blockIdx.x * 4);
 }
 
-// E_slot[slot] = -sum_z partial[slot][z][0] ; M_slot[slot][mu] = (1/N) sum_z partial[slot][z][1+mu]   (fixed order)
-__global__ void finalize_energy_kernel(Geom g, const double* __restrict__ partial, double* __restrict__ e_slot, double* __restrict__ m_slot) {
+// E_slot[slot] = -sum_chunks partial[slot][chunk][0] ; M_slot[slot][mu] = (1/N) sum_chunks partial[slot][chunk][1+mu]   (fixed order)
+__global__ void finalize_energy_kernel(Geom g, int n_chunks, const double* __restrict__ partial, double* __restrict__ e_slot, double* __restrict__ m_slot) {
   const int tid = blockIdx.x * kThreads + threadIdx.x;
   if (tid >= g.R * 4) return;
   const int slot = tid / 4, k = tid % 4;
   double x = 0.0;
-  for (int z = 0; z < g.L; ++z) x += partial[((long long)slot * g.L + z) * 4 + k];
+  for (int z = 0; z < n_chunks; ++z) x += partial[((long long)slot * n_chunks + z) * 4 + k];
   if (k == 0) e_slot[slot] = -x;
   else m_slot[slot * 3 + (k - 1)] = x / (double)g.N;
 }
@@ -321,13 +346,16 @@ __global__ void pt_swap_kernel(Geom g, PhiloxKey key, unsigned long long k_pt, c
 }
 
 // ------------------------------------------------------------------ overlap tensor, Eqs. (5), (6)
-// One block per (d, pair, t, z-plane): partial[(d,p,t)][z][27] = 9 sums for k=0, 9 re, 9 im for k_min.
-__global__ void __launch_bounds__(kThreads) overlap_kernel(Geom g, const float* __restrict__ spins, const int32_t* __restrict__ slot_of_temp,
+// One block per (d, pair, t, chunk of ZB planes): partial[(d,p,t)][chunk][27] = 9 sums for k=0, 9 re, 9 im
+// for k_min.  Each thread takes items of V compact sites (vector loads of both replicas).
+template <int V>
+__global__ void __launch_bounds__(kThreads) overlap_kernel(Geom g, int ZB, const float* __restrict__ spins, const int32_t* __restrict__ slot_of_temp,
                                                            const double* __restrict__ cs_table /*[L][2]*/, double* __restrict__ partial) {
-  const int L = g.L, Lh = g.Lh;
+  const int L = g.L, Lh = g.Lh, qpr = Lh / V;
   const int P = g.O * (g.O - 1) / 2;
-  const int z = blockIdx.x % L;
-  int rest = blockIdx.x / L;                // (d*P + p)*T + t
+  const int n_chunks = (L + ZB - 1) / ZB;
+  const int chunk = blockIdx.x % n_chunks;
+  int rest = blockIdx.x / n_chunks;         // (d*P + p)*T + t
   const int t = rest % g.T; rest /= g.T;
   const int p = rest % P; const int d = rest / P;
   int a = 0, b = 1;
@@ -336,46 +364,83 @@ __global__ void __launch_bounds__(kThreads) overlap_kernel(Geom g, const float* 
   const int sb = (d * g.O + b) * g.T + slot_of_temp[(d * g.O + b) * g.T + t];
   const float* A = spins + (long long)sa * 3 * g.N;
   const float* B = spins + (long long)sb * 3 * g.N;
+  const int z0 = chunk * ZB, nz = min(ZB, L - z0);
   double acc[27];
 #pragma unroll
   for (int k = 0; k < 27; ++k) acc[k] = 0.0;
-  const int per_plane = 2 * L * Lh;
-  for (int idx = threadIdx.x; idx < per_plane; idx += kThreads) {
-    const int j = idx % Lh; int rem = idx / Lh;
-    const int y = rem % L; const int c = rem / L;
-    const int x = 2 * j + ((y + z + c) & 1);
-    const double co = cs_table[2 * x], si = cs_table[2 * x + 1];
-    double sa3[3], sb3[3];
+  const int ipp = 2 * L * qpr;
+  for (int it = threadIdx.x; it < nz * ipp; it += kThreads) {
+    const int q = it % qpr; int rem = it / qpr;
+    const int y = rem % L; rem /= L;
+    const int c = rem & 1; const int z = z0 + (rem >> 1);
+    const int j0 = q * V;
+    const int off = (y + z + c) & 1;
+    Vec<V> av[3], bv[3];
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) {
-      sa3[mu] = (double)A[spin_index(g, z, c, mu, y, j)];
-      sb3[mu] = (double)B[spin_index(g, z, c, mu, y, j)];
+      av[mu] = ldv<V>(A + spin_index(g, z, c, mu, y, j0));
+      bv[mu] = ldv<V>(B + spin_index(g, z, c, mu, y, j0));
     }
 #pragma unroll
-    for (int mu = 0; mu < 3; ++mu)
+    for (int e = 0; e < V; ++e) {
+      const int x = 2 * (j0 + e) + off;
+      const double co = cs_table[2 * x], si = cs_table[2 * x + 1];
+      double ad[3], bd[3], bc[3], bs[3];
 #pragma unroll
-      for (int nu = 0; nu < 3; ++nu) {
-        const double pr = sa3[mu] * sb3[nu];
-        acc[mu * 3 + nu] += pr;
-        acc[9 + mu * 3 + nu] = fma(pr, co, acc[9 + mu * 3 + nu]);
-        acc[18 + mu * 3 + nu] = fma(pr, si, acc[18 + mu * 3 + nu]);
-      }
+      for (int mu = 0; mu < 3; ++mu) { ad[mu] = (double)av[mu].v[e]; bd[mu] = (double)bv[mu].v[e]; bc[mu] = bd[mu] * co; bs[mu] = bd[mu] * si; }
+#pragma unroll
+      for (int mu = 0; mu < 3; ++mu)
+#pragma unroll
+        for (int nu = 0; nu < 3; ++nu) {
+          acc[mu * 3 + nu] = fma(ad[mu], bd[nu], acc[mu * 3 + nu]);
+          acc[9 + mu * 3 + nu] = fma(ad[mu], bc[nu], acc[9 + mu * 3 + nu]);
+          acc[18 + mu * 3 + nu] = fma(ad[mu], bs[nu], acc[18 + mu * 3 + nu]);
+        }
+    }
   }
   block_reduce_store<27>(acc, partial + (long long)blockIdx.x * 27);
 }
 
-__global__ void finalize_overlap_kernel(Geom g, int n_sys /*D*P*T*/, const double* __restrict__ partial, double* __restrict__ q0, double* __restrict__ qk) {
+__global__ void finalize_overlap_kernel(Geom g, int n_sys /*D*P*T*/, int n_chunks, const double* __restrict__ partial, double* __restrict__ q0, double* __restrict__ qk) {
   const int tid = blockIdx.x * kThreads + threadIdx.x;
   if (tid >= n_sys * 9) return;
   const int sys = tid / 9, k = tid % 9;
   double r0 = 0.0, re = 0.0, im = 0.0;
-  for (int z = 0; z < g.L; ++z) {
-    const double* p = partial + ((long long)sys * g.L + z) * 27;
+  for (int z = 0; z < n_chunks; ++z) {
+    const double* p = partial + ((long long)sys * n_chunks + z) * 27;
     r0 += p[k]; re += p[9 + k]; im += p[18 + k];
   }
   const double inv = 1.0 / (double)g.N;
   if (q0) q0[tid] = r0 * inv;
   if (qk) { qk[2 * tid] = re * inv; qk[2 * tid + 1] = im * inv; }
+}
+
+// ------------------------------------------------------------------ arithmetic self-test (hsg_selftest_arith)
+// Compares div_rn / sqrt_rn with the compiler's IEEE __fdiv_rn / __fsqrt_rn on pseudo-random operands whose
+// exponents cover [2^-100, 2^100] (all mantissa bits random); counts[0] = division mismatches,
+// counts[1] = square-root mismatches.
+__global__ void selftest_arith_kernel(PhiloxKey key, unsigned long long n, unsigned long long* __restrict__ counts) {
+  const unsigned long long tid = (unsigned long long)blockIdx.x * kThreads + threadIdx.x;
+  const unsigned long long stride = (unsigned long long)gridDim.x * kThreads;
+  unsigned int bad_div = 0, bad_sqrt = 0;
+  for (unsigned long long i = tid; i < n; i += stride) {
+    uint32_t w0, w1, w2, w3;
+    philox4x32_10((uint32_t)i, (uint32_t)(i >> 32), 0x5e1f7e57u, 0u, key.k0, key.k1, w0, w1, w2, w3);
+    const uint32_t ea = 27u + (w2 % 201u), eb = 27u + ((w2 >> 8) % 201u);            // biased exponents 27..227
+    const float a = __uint_as_float((w0 & 0x807FFFFFu) | (ea << 23));
+    const float b = __uint_as_float((w1 & 0x807FFFFFu) | (eb << 23));
+    const float x = fabsf(b);
+    const float q1 = div_rn(a, b), q2 = __fdiv_rn(a, b);
+    // the quotient itself must stay a normal number for the comparison to be in the supported range
+    if (fabsf(q2) >= 1.2e-38f && fabsf(q2) <= 3.0e38f && __float_as_uint(q1) != __float_as_uint(q2)) ++bad_div;
+    if (__float_as_uint(sqrt_rn(x)) != __float_as_uint(__fsqrt_rn(x))) ++bad_sqrt;
+    // operands shaped like the moves': a denominator in [1, 3), a numerator of order one
+    const float b2 = __uint_as_float((w1 & 0x007FFFFFu) | (127u << 23)) + (float)(w3 & 1u);
+    const float a2 = __uint_as_float((w3 & 0x807FFFFFu) | ((120u + (w3 >> 28)) << 23));
+    if (__float_as_uint(div_rn(a2, b2)) != __float_as_uint(__fdiv_rn(a2, b2))) ++bad_div;
+  }
+  if (bad_div) atomicAdd(counts, (unsigned long long)bad_div);
+  if (bad_sqrt) atomicAdd(counts + 1, (unsigned long long)bad_sqrt);
 }
 
 }  // namespace hsg

@@ -44,42 +44,31 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)_
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
 
 // ---------------------------------------------------------------- V-wide vector access (V = 2 or 4 floats)
 template <int V> struct VT;
 template <> struct VT<2> { using type = float2; };
 template <> struct VT<4> { using type = float4; };
 
-template <int V> __device__ __forceinline__ void ld(float (&r)[V], const float* p) {
-  const typename VT<V>::type t = *reinterpret_cast<const typename VT<V>::type*>(p);
-  const float* f = reinterpret_cast<const float*>(&t);
-#pragma unroll
-  for (int e = 0; e < V; ++e) r[e] = f[e];
+// shared memory by 32-bit shared-window byte address (keeps all address arithmetic 32-bit)
+template <int V> __device__ __forceinline__ void lds(float (&r)[V], uint32_t a);
+template <> __device__ __forceinline__ void lds<2>(float (&r)[2], uint32_t a) {
+  asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(r[0]), "=f"(r[1]) : "r"(a) : "memory");
 }
-template <int V> __device__ __forceinline__ void st(float* p, const float (&r)[V]) {
-  typename VT<V>::type t;
-  float* f = reinterpret_cast<float*>(&t);
-#pragma unroll
-  for (int e = 0; e < V; ++e) f[e] = r[e];
-  *reinterpret_cast<typename VT<V>::type*>(p) = t;
+template <> __device__ __forceinline__ void lds<4>(float (&r)[4], uint32_t a) {
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]) : "r"(a) : "memory");
+}
+__device__ __forceinline__ float lds1(uint32_t a) {
+  float r;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(a) : "memory");
+  return r;
+}
+template <int V> __device__ __forceinline__ void sts(uint32_t a, const float (&r)[V]);
+template <> __device__ __forceinline__ void sts<2>(uint32_t a, const float (&r)[2]) {
+  asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(a), "f"(r[0]), "f"(r[1]) : "memory");
+}
+template <> __device__ __forceinline__ void sts<4>(uint32_t a, const float (&r)[4]) {
+  asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]) : "memory");
 }
 // streaming global access for the spins: each value is touched once per sweep
 template <int V> __device__ __forceinline__ void ldg(float (&r)[V], const float* p) {
@@ -104,53 +93,58 @@ template <int L, int V, int G> struct Cfg {
   static constexpr int CS = L * Lh;               // one [y][j] array
   static constexpr int HP = 3 * CS;               // spin half-plane (one colour, 3 components)
   static constexpr int JP = 12 * CS;              // J/H plane (2 colours x 6 arrays)
-  static constexpr size_t smem_bytes = 64 + sizeof(float) * ((size_t)kRing * JP + (size_t)G * 4 * HP);
+  static constexpr uint32_t ring_off = 64;        // byte offsets inside dynamic shared memory
+  static constexpr uint32_t x_off = ring_off + 4u * kRing * JP;
+  static constexpr size_t smem_bytes = x_off + sizeof(float) * ((size_t)G * 4 * HP);
   static_assert(Lh % V == 0, "row length must be a multiple of the vector width");
   static_assert((JP * 4) % 16 == 0, "bulk copies move multiples of 16 bytes");
 };
 
-// per-thread constants of the march
+// per-thread constants of the march (byte offsets inside a [y][j] array)
 struct Th {
   int y, j0;
-  int row, rowp, rowm;     // float offsets inside a [y][j] array: own row, row y+1, row y-1 (periodic) at j0
-  int edge0, edge1;        // own row at j0-1 and j0+V (periodic): the x neighbour outside the thread's V sites
+  uint32_t row, rowp, rowm;   // own row, row y+1, row y-1 (periodic) at j0
+  uint32_t edge0, edge1;      // own row at j0-1 and j0+V (periodic): the x neighbour outside the thread's V sites
 };
+
+struct HbPar { float beta; uint32_t sysid, c1, c3; PhiloxKey key; };
 
 // Local field of V sites of colour `cu` in plane zp, accumulated in the order H, x+, x-, y+, y-, z+, z-
 // (DESIGN.md §3.1), then the move.  `q` = the thread's own column of the other colour in this plane,
 // `xs` = shared-memory half-plane of the other colour in this plane (rows y+-1 and the x edge),
 // `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1,
 // `jo` = J/H arrays of colour cu in plane zp, `jx` = arrays of the other colour in plane zp,
-// `jzlo` = Jz array of the other colour in plane zp-1 (all in the shared-memory ring).
+// `jzlo` = Jz array of the other colour in plane zp-1 (shared-memory ring; all 32-bit shared addresses).
 template <int L, int V, bool HB>
 __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&own)[3][V], const float (&q)[3][V],
-                                             const float (&zlo)[3][V], const float (&zhi)[3][V], const float* __restrict__ xs,
-                                             const float* __restrict__ jo, const float* __restrict__ jx, const float* __restrict__ jzlo,
-                                             const Th& th, int off, float beta, uint32_t sysid, uint32_t c1, uint32_t c3,
-                                             PhiloxKey key, uint32_t site0) {
-  constexpr int CS = L * (L / 2);
-  const int edge = off ? th.edge1 : th.edge0;
+                                             const float (&zlo)[3][V], const float (&zhi)[3][V], uint32_t xs,
+                                             uint32_t jo, uint32_t jx, uint32_t jzlo,
+                                             const Th& th, int off, const HbPar& hp, uint32_t site0) {
+  constexpr uint32_t CSB = 4u * L * (L / 2);
+  const uint32_t edge = off ? th.edge1 : th.edge0;
   float Jxp[V], Jxm[V], Jyp[V], Jym[V], Jzp[V], Jzm[V];
-  ld<V>(Jxp, jo + 0 * CS + th.row);
-  ld<V>(Jyp, jo + 1 * CS + th.row);
-  ld<V>(Jzp, jo + 2 * CS + th.row);
+  const uint32_t jo_row = jo + th.row;
+  lds<V>(Jxp, jo_row);
+  lds<V>(Jyp, jo_row + CSB);
+  lds<V>(Jzp, jo_row + 2 * CSB);
   {
     float t[V];
-    ld<V>(t, jx + 0 * CS + th.row);
-    const float te = jx[0 * CS + th.edge0];
+    lds<V>(t, jx + th.row);
+    const float te = lds1(jx + th.edge0);
 #pragma unroll
     for (int e = 0; e < V; ++e) Jxm[e] = off ? t[e] : (e > 0 ? t[e > 0 ? e - 1 : 0] : te);
   }
-  ld<V>(Jym, jx + 1 * CS + th.rowm);
-  ld<V>(Jzm, jzlo + th.row);
+  lds<V>(Jym, jx + CSB + th.rowm);
+  lds<V>(Jzm, jzlo + th.row);
   float h[3][V];
+  const uint32_t xs_p = xs + th.rowp, xs_m = xs + th.rowm, xs_e = xs + edge;
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
     float Hm[V], yp[V], ym[V];
-    ld<V>(Hm, jo + (3 + mu) * CS + th.row);
-    ld<V>(yp, xs + mu * CS + th.rowp);
-    ld<V>(ym, xs + mu * CS + th.rowm);
-    const float se = xs[mu * CS + edge];
+    lds<V>(Hm, jo_row + (3 + mu) * CSB);
+    lds<V>(yp, xs_p + mu * CSB);
+    lds<V>(ym, xs_m + mu * CSB);
+    const float se = lds1(xs_e + mu * CSB);
 #pragma unroll
     for (int e = 0; e < V; ++e) {
       const float sxp = off ? (e + 1 < V ? q[mu][e + 1 < V ? e + 1 : 0] : se) : q[mu][e];
@@ -171,8 +165,8 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
     Vec3 s;
     if (HB) {
       uint32_t w0, w1, w2, w3;
-      philox4x32_10(site0 + 2u * (uint32_t)e, c1, sysid, c3, key.k0, key.k1, w0, w1, w2, w3);
-      s = hb_draw(hv, beta, u01(w0), u01(w1));
+      philox4x32_10(site0 + 2u * (uint32_t)e, hp.c1, hp.sysid, hp.c3, hp.key.k0, hp.key.k1, w0, w1, w2, w3);
+      s = hb_draw(hv, hp.beta, u01(w0), u01(w1));
     } else {
       const Vec3 sv = {own[0][e], own[1][e], own[2][e]};
       s = or_reflect(sv, hv);
@@ -181,92 +175,113 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
   }
 }
 
-// Shared state of one CTA during the march
-template <int L, int V, int G> struct Smem {
-  using C = Cfg<L, V, G>;
-  uint64_t* full;      // [kRing] mbarriers
-  float* ring;         // [kRing][JP]
-  float* x0;           // this thread's system: [2][HP] new colour-0 spins of planes k-1, k
-  float* x1;           // this thread's system: [2][HP] old colour-1 spins of planes k, k+1
+// Shared state of one CTA during the march (32-bit shared-window addresses)
+struct Smem {
+  uint32_t full;       // [kRing] mbarriers
+  uint32_t ring;       // [kRing][JP] floats
+  uint32_t x0;         // this thread's system: [2][HP] new colour-0 spins of planes k-1, k
+  uint32_t x1;         // this thread's system: [2][HP] old colour-1 spins of planes k, k+1
 };
+
+struct Stream {        // J/H plane stream: index q -> plane (q-1) mod L
+  int issued, waited, total;
+};
+
+template <int L, int JP>
+__device__ __forceinline__ void ring_advance(const Smem& sm, const float* __restrict__ jh_d, Stream& st, int nd) {
+  if (threadIdx.x == 0) {                               // producer: keep one plane in flight
+    const int upto = min(nd + 1, st.total - 1);
+    while (st.issued < upto) {
+      ++st.issued;
+      const int plane = (st.issued + L - 1) % L;
+      const uint32_t slot = (uint32_t)st.issued % kRing;
+      const uint32_t bar = sm.full + 8u * slot;
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((uint32_t)JP * 4u) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(sm.ring + slot * (uint32_t)JP * 4u), "l"(jh_d + (size_t)plane * JP), "r"((uint32_t)JP * 4u), "r"(bar) : "memory");
+    }
+  }
+  while (st.waited < nd) {
+    ++st.waited;
+    const uint32_t bar = sm.full + 8u * ((uint32_t)st.waited % kRing);
+    const uint32_t parity = ((uint32_t)st.waited / kRing) & 1u;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+  }
+}
 
 // One full sweep (both colours, all planes) of the G systems of this CTA.
 template <int L, int V, int G, bool HB>
-__device__ __forceinline__ void march_sweep(const Smem<L, V, G>& sm, float* __restrict__ S, const float* __restrict__ jh_d,
-                                            const Th& th, float beta, uint32_t sysid, unsigned long long khb, PhiloxKey key,
-                                            int qbase, int total, int& issued, int& waited) {
+__device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ S, const float* __restrict__ jh_d,
+                                            const Th& th, const HbPar& hp, int qbase, Stream& st) {
   using C = Cfg<L, V, G>;
   constexpr int CS = C::CS, HP = C::HP, JP = C::JP, PS = 2 * C::HP;
-  const uint32_t c1 = (uint32_t)(khb & 0xFFFFFFFFull), c3 = counter_hi(khb, DOMAIN_HB);
+  constexpr uint32_t CSB = 4u * CS, HPB = 4u * HP, JPB = 4u * JP;
   float A[3][V], B[3][V], Cc[3][V], O[3][V], P[3][V], Q[3][V], R[3][V], Cn[3][V], On[3][V];
+  float* Sr = S + (th.row >> 2);                       // own column, plane 0, colour 0, component 0
   // prologue: A = c1old(L-1), B = c1old(0) (published in X1[0]), prefetch c1old(1) and c0old(0)
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
-    ldg<V>(A[mu], S + (L - 1) * PS + HP + mu * CS + th.row);
-    ldg<V>(B[mu], S + HP + mu * CS + th.row);
-    ldg<V>(Cn[mu], S + 1 * PS + HP + mu * CS + th.row);
-    if (!HB) ldg<V>(On[mu], S + mu * CS + th.row);
+    ldg<V>(A[mu], Sr + (L - 1) * PS + HP + mu * CS);
+    ldg<V>(B[mu], Sr + HP + mu * CS);
+    ldg<V>(Cn[mu], Sr + 1 * PS + HP + mu * CS);
+    if (!HB) ldg<V>(On[mu], Sr + mu * CS);
 #pragma unroll
     for (int e = 0; e < V; ++e) { P[mu][e] = 0.0f; Q[mu][e] = 0.0f; if (HB) On[mu][e] = 0.0f; }
-    st<V>(sm.x1 + mu * CS + th.row, B[mu]);
+    sts<V>(sm.x1 + mu * CSB + th.row, B[mu]);
   }
   __syncthreads();
-#pragma unroll 1
-  for (int k = 0; k < L + 2; ++k) {
-    const int nd = qbase + (k < L ? k + 1 : k);           // newest J/H stream index this step reads
-    if (threadIdx.x == 0) {                               // producer: keep one plane in flight
-      const int upto = min(nd + 1, total - 1);
-      while (issued < upto) {
-        ++issued;
-        const int plane = (issued + L - 1) % L;
-        uint64_t* bar = sm.full + (issued % kRing);
-        mbar_expect_tx(bar, JP * 4);
-        bulk_g2s(sm.ring + (issued % kRing) * JP, jh_d + (size_t)plane * JP, JP * 4, bar);
-      }
-    }
+  // main steps: colour 0 of plane k, then colour 1 of plane k-1
+#pragma unroll 2
+  for (int k = 0; k < L; ++k) {
+    const int nd = qbase + k + 1;                       // newest J/H stream index this step reads (plane k)
+    ring_advance<L, JP>(sm, jh_d, st, nd);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
       for (int e = 0; e < V; ++e) { Cc[mu][e] = Cn[mu][e]; O[mu][e] = On[mu][e]; }
-    if (k + 1 < L) {
+    if (k + 1 < L) {                                    // prefetch the next step's planes
       const int zc = (k + 2 == L) ? 0 : k + 2;
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) {
-        ldg<V>(Cn[mu], S + zc * PS + HP + mu * CS + th.row);
-        if (!HB) ldg<V>(On[mu], S + (k + 1) * PS + mu * CS + th.row);
+        ldg<V>(Cn[mu], Sr + zc * PS + HP + mu * CS);
+        if (!HB) ldg<V>(On[mu], Sr + (k + 1) * PS + mu * CS);
+      }
+    } else {                                            // k = L-1: the new colour 0 of plane 0, needed by step L
+#pragma unroll
+      for (int mu = 0; mu < 3; ++mu) ldg<V>(On[mu], Sr + mu * CS);
+    }
+    const int off = (th.y + k) & 1;
+    const uint32_t jk = sm.ring + ((uint32_t)nd % kRing) * JPB;                  // plane k
+    const uint32_t jk1 = sm.ring + ((uint32_t)(nd + kRing - 1) % kRing) * JPB;   // plane k-1
+    const uint32_t jk2 = sm.ring + ((uint32_t)(nd + kRing - 2) % kRing) * JPB;   // plane k-2
+    const uint32_t par = (uint32_t)(k & 1);
+    {
+      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * k));
+      update_sites<L, V, HB>(R, O, B, A, Cc, sm.x1 + par * HPB, jk, jk + 6 * CSB, jk1 + 8 * CSB, th, off, hp, site0);
+#pragma unroll
+      for (int mu = 0; mu < 3; ++mu) {
+        stg<V>(Sr + k * PS + mu * CS, R[mu]);
+        sts<V>(sm.x0 + par * HPB + mu * CSB + th.row, R[mu]);
       }
     }
-    while (waited < nd) { ++waited; mbar_wait(sm.full + (waited % kRing), (uint32_t)(waited / kRing) & 1u); }
-    const int off = (th.y + k) & 1;
-    const float* jk = sm.ring + (nd % kRing) * JP;                 // k < L: plane k;   k >= L: plane k-1
-    const float* jk1 = sm.ring + ((nd - 1) % kRing) * JP;
-    const float* jk2 = sm.ring + ((nd - 2 + kRing) % kRing) * JP;
-    if (k < L) {
-      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * k));
-      update_sites<L, V, HB>(R, O, B, A, Cc, sm.x1 + (k & 1) * HP, jk, jk + 6 * CS, jk1 + 8 * CS, th, off, beta, sysid, c1, c3, key, site0);
-#pragma unroll
-      for (int mu = 0; mu < 3; ++mu) stg<V>(S + k * PS + mu * CS + th.row, R[mu]);
-    } else {
-#pragma unroll
-      for (int mu = 0; mu < 3; ++mu) ldg<V>(R[mu], S + (k - L) * PS + mu * CS + th.row);   // new colour 0 of planes 0, 1
-    }
-    if (k <= L) {
-#pragma unroll
-      for (int mu = 0; mu < 3; ++mu) st<V>(sm.x0 + (k & 1) * HP + mu * CS + th.row, R[mu]);
-    }
-    if (k >= 2) {     // colour 1 of plane k-1 (plane 0 when k = L+1)
-      const int z1 = (k - 1 == L) ? 0 : k - 1;
-      const float* j1 = (k < L) ? jk1 : jk;          // plane k-1
-      const float* j2 = (k < L) ? jk2 : jk1;         // plane k-2
-      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * z1));
+    if (k >= 2) {     // colour 1 of plane k-1
+      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * (k - 1)));
       float N1[3][V];
-      update_sites<L, V, HB>(N1, A, Q, P, R, sm.x0 + ((k - 1) & 1) * HP, j1 + 6 * CS, j1, j2 + 2 * CS, th, off, beta, sysid, c1, c3, key, site0);
+      update_sites<L, V, HB>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, jk1 + 6 * CSB, jk1, jk2 + 2 * CSB, th, off, hp, site0);
 #pragma unroll
-      for (int mu = 0; mu < 3; ++mu) stg<V>(S + z1 * PS + HP + mu * CS + th.row, N1[mu]);
+      for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + (k - 1) * PS + HP + mu * CS, N1[mu]);
     }
     if (k + 1 < L) {
 #pragma unroll
-      for (int mu = 0; mu < 3; ++mu) st<V>(sm.x1 + ((k + 1) & 1) * HP + mu * CS + th.row, Cc[mu]);
+      for (int mu = 0; mu < 3; ++mu) sts<V>(sm.x1 + (par ^ 1u) * HPB + mu * CSB + th.row, Cc[mu]);
     }
     __syncthreads();
 #pragma unroll
@@ -274,50 +289,92 @@ __device__ __forceinline__ void march_sweep(const Smem<L, V, G>& sm, float* __re
 #pragma unroll
       for (int e = 0; e < V; ++e) { A[mu][e] = B[mu][e]; B[mu][e] = Cc[mu][e]; P[mu][e] = Q[mu][e]; Q[mu][e] = R[mu][e]; }
   }
+  // tail: colour 1 of plane L-1 (step L) and of plane 0 (step L+1); their z+ neighbours are the new colour-0
+  // spins of planes 0 and 1, read back from the thread's own column
+#pragma unroll 1
+  for (int kk = 0; kk < 2; ++kk) {
+    const int k = L + kk;
+    const int nd = qbase + k;                            // plane k-1 (mod L)
+    ring_advance<L, JP>(sm, jh_d, st, nd);
+#pragma unroll
+    for (int mu = 0; mu < 3; ++mu)
+#pragma unroll
+      for (int e = 0; e < V; ++e) R[mu][e] = On[mu][e];
+    if (kk == 0) {
+#pragma unroll
+      for (int mu = 0; mu < 3; ++mu) {
+        ldg<V>(On[mu], Sr + PS + mu * CS);               // new colour 0 of plane 1, needed by step L+1
+        sts<V>(sm.x0 + mu * CSB + th.row, R[mu]);         // L is even: X0[L & 1] = X0[0] <- new colour 0 of plane 0
+      }
+    }
+    const int off = (th.y + k) & 1;
+    const uint32_t j1 = sm.ring + ((uint32_t)nd % kRing) * JPB;                  // plane k-1
+    const uint32_t j2 = sm.ring + ((uint32_t)(nd + kRing - 1) % kRing) * JPB;    // plane k-2
+    const int z1 = kk == 0 ? L - 1 : 0;
+    const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * z1));
+    float N1[3][V];
+    update_sites<L, V, HB>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, j1 + 6 * CSB, j1, j2 + 2 * CSB, th, off, hp, site0);
+#pragma unroll
+    for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + z1 * PS + HP + mu * CS, N1[mu]);
+    __syncthreads();
+#pragma unroll
+    for (int mu = 0; mu < 3; ++mu)
+#pragma unroll
+      for (int e = 0; e < V; ++e) { A[mu][e] = B[mu][e]; P[mu][e] = Q[mu][e]; Q[mu][e] = R[mu][e]; }
+  }
 }
 
 template <int L, int V, int G>
 __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs a) {
   using C = Cfg<L, V, G>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  Smem<L, V, G> sm;
-  sm.full = reinterpret_cast<uint64_t*>(smem_raw);
-  sm.ring = reinterpret_cast<float*>(smem_raw + 64);
-  float* xbase = sm.ring + kRing * C::JP;
+  const uint32_t base = smem_u32(smem_raw);
   const int gs = threadIdx.x / C::TPS, tl = threadIdx.x % C::TPS;
-  sm.x0 = xbase + (gs * 4) * C::HP;
-  sm.x1 = xbase + (gs * 4 + 2) * C::HP;
+  Smem sm;
+  sm.full = base;
+  sm.ring = base + C::ring_off;
+  sm.x0 = base + C::x_off + 4u * (uint32_t)(gs * 4) * C::HP;
+  sm.x1 = sm.x0 + 4u * 2 * C::HP;
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int i = 0; i < kRing; ++i) mbar_init(sm.full + i, 1);
+    for (int i = 0; i < kRing; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
   Th th;
   th.y = tl / C::TPR; th.j0 = (tl % C::TPR) * V;
-  th.row = th.y * C::Lh + th.j0;
-  th.rowp = ((th.y + 1 == L) ? 0 : th.y + 1) * C::Lh + th.j0;
-  th.rowm = ((th.y == 0) ? L - 1 : th.y - 1) * C::Lh + th.j0;
-  th.edge0 = th.y * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1);
-  th.edge1 = th.y * C::Lh + ((th.j0 + V == C::Lh) ? 0 : th.j0 + V);
+  th.row = 4u * (uint32_t)(th.y * C::Lh + th.j0);
+  th.rowp = 4u * (uint32_t)(((th.y + 1 == L) ? 0 : th.y + 1) * C::Lh + th.j0);
+  th.rowm = 4u * (uint32_t)(((th.y == 0) ? L - 1 : th.y - 1) * C::Lh + th.j0);
+  th.edge0 = 4u * (uint32_t)(th.y * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1));
+  th.edge1 = 4u * (uint32_t)(th.y * C::Lh + ((th.j0 + V == C::Lh) ? 0 : th.j0 + V));
 
   const Geom& g = a.g;
   const int slot = blockIdx.x * G + gs;                 // G consecutive slots of one sample
   const int d = slot / (g.O * g.T);
   const int grp = slot / g.T;
   const int t = a.temp_of_slot[slot];
-  const float beta = a.beta[t];
-  const uint32_t sysid = (uint32_t)((g.sample_offset * g.O * g.T) + (unsigned long long)grp * g.T + t);
+  HbPar hp;
+  hp.beta = a.beta[t];
+  hp.sysid = (uint32_t)((g.sample_offset * g.O * g.T) + (unsigned long long)grp * g.T + t);
+  hp.key = a.key;
   float* S = a.spins + (size_t)slot * 3 * g.N;
   const float* jh_d = a.jh + (size_t)d * 6 * g.N;
 
   const int n_sweeps = a.n_or + a.n_hb;
-  const int total = n_sweeps * L + 2;                   // J/H stream: planes L-1, 0, 1, ..., repeated; index q -> plane (q-1) mod L
-  int issued = -1, waited = -1;
+  Stream st;
+  st.issued = -1; st.waited = -1;
+  st.total = n_sweeps * L + 2;                          // planes L-1, 0, 1, ..., L-1, 0, 1, ... (index q -> plane (q-1) mod L)
   for (int s = 0; s < n_sweeps; ++s) {
-    if (s < a.n_or) march_sweep<L, V, G, false>(sm, S, jh_d, th, beta, sysid, 0ull, a.key, s * L, total, issued, waited);
-    else march_sweep<L, V, G, true>(sm, S, jh_d, th, beta, sysid, a.k_hb + (unsigned long long)(s - a.n_or), a.key, s * L, total, issued, waited);
+    if (s < a.n_or) {
+      hp.c1 = 0; hp.c3 = 0;
+      march_sweep<L, V, G, false>(sm, S, jh_d, th, hp, s * L, st);
+    } else {
+      const unsigned long long khb = a.k_hb + (unsigned long long)(s - a.n_or);
+      hp.c1 = (uint32_t)(khb & 0xFFFFFFFFull); hp.c3 = counter_hi(khb, DOMAIN_HB);
+      march_sweep<L, V, G, true>(sm, S, jh_d, th, hp, s * L, st);
+    }
   }
 }
 

@@ -234,3 +234,10 @@ def test_zero_local_field_is_handled():
     eng.sweep(0, 1); orc.sweep(0, 1)
     assert np.array_equal(_spins(eng), orc.get_spins())
     assert np.isfinite(_spins(eng)).all()
+
+
+def test_branch_free_division_and_sqrt_are_ieee_correct():
+    """The kernels' div_rn / sqrt_rn against the compiler's correctly rounded division and square root,
+    2e8 operand sets with random mantissas and exponents over [2^-100, 2^100]."""
+    import paper_1204_6192_b200 as hsg
+    assert hsg.hsg_selftest_arith(200_000_000, seed=12345) == (0, 0)
