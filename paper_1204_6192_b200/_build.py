@@ -44,6 +44,9 @@ def stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
+    override = os.environ.get("HSG_LIB")          # experiments: load a pre-built variant instead
+    if override:
+        return Path(override)
     if not force and not stale():
         return LIB
     LIB.parent.mkdir(parents=True, exist_ok=True)

@@ -37,7 +37,20 @@ struct ZmarchArgs {
 
 namespace zm {
 
-constexpr int kRing = 4;   // J/H ring slots: planes k-2, k-1, k live + plane k+1 in flight
+#ifndef HSG_ZM_UNROLL
+#define HSG_ZM_UNROLL 2
+#endif
+#ifndef HSG_ZM_L32_V
+#define HSG_ZM_L32_V 2
+#endif
+#ifndef HSG_ZM_L32_G
+#define HSG_ZM_L32_G 2
+#endif
+#ifndef HSG_ZM_L16_V
+#define HSG_ZM_L16_V 2
+#endif
+constexpr int kRing = 4;
+constexpr int kUnroll = HSG_ZM_UNROLL;   // unroll factor of the main march loop   // J/H ring slots: planes k-2, k-1, k live + plane k+1 in flight
 
 // ---------------------------------------------------------------- PTX wrappers: mbarrier + bulk async copy
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -239,7 +252,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   }
   __syncthreads();
   // main steps: colour 0 of plane k, then colour 1 of plane k-1
-#pragma unroll 2
+#pragma unroll kUnroll
   for (int k = 0; k < L; ++k) {
     const int nd = qbase + k + 1;                       // newest J/H stream index this step reads (plane k)
     ring_advance<L, JP>(sm, jh_d, st, nd);
@@ -409,11 +422,17 @@ inline bool zmarch_supported(const Geom& g) { return g.L == 8 || g.L == 16 || g.
 inline cudaError_t zmarch_launch(const ZmarchArgs& a, cudaStream_t stream, int* n_launch) {
   *n_launch = 1;
   if (a.g.L == 32) {
-    const int G = zmarch_pick_g(a.g, 4);
-    HSG_ZM_CASE(32, 4, 4) HSG_ZM_CASE(32, 4, 2) HSG_ZM_CASE(32, 4, 1)
+    const int G = zmarch_pick_g(a.g, HSG_ZM_L32_G);
+    HSG_ZM_CASE(32, HSG_ZM_L32_V, HSG_ZM_L32_G)
+#if HSG_ZM_L32_G > 2
+    HSG_ZM_CASE(32, HSG_ZM_L32_V, 2)
+#endif
+#if HSG_ZM_L32_G > 1
+    HSG_ZM_CASE(32, HSG_ZM_L32_V, 1)
+#endif
   } else if (a.g.L == 16) {
     const int G = zmarch_pick_g(a.g, 8);
-    HSG_ZM_CASE(16, 4, 8) HSG_ZM_CASE(16, 4, 4) HSG_ZM_CASE(16, 4, 2) HSG_ZM_CASE(16, 4, 1)
+    HSG_ZM_CASE(16, HSG_ZM_L16_V, 8) HSG_ZM_CASE(16, HSG_ZM_L16_V, 4) HSG_ZM_CASE(16, HSG_ZM_L16_V, 2) HSG_ZM_CASE(16, HSG_ZM_L16_V, 1)
   } else if (a.g.L == 8) {
     const int G = zmarch_pick_g(a.g, 8);
     HSG_ZM_CASE(8, 2, 8) HSG_ZM_CASE(8, 2, 4) HSG_ZM_CASE(8, 2, 2) HSG_ZM_CASE(8, 2, 1)
