@@ -168,6 +168,8 @@ def main_ours(args, cfg, temps):
     H = hsg_inputs.gaussian_field(L, D, cfg["h_r"], cfg["seed"], off) if cfg["h_r"] > 0 else None
 
     eng = hsg.hsg_create(L, D, O, temps, cfg["seed"], sample_offset=off, kernel=args.kernel)
+    if args.no_fuse_energy:
+        eng.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
     eng.set_disorder(J, H)
     eng.init_spins()
     f64, i32 = torch.float64, torch.int32
@@ -309,6 +311,7 @@ def main():
     ap.add_argument("--samples", type=int, default=None, help="override the number of disorder samples per GPU")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-measure", action="store_true")
+    ap.add_argument("--no-fuse-energy", action="store_true", help="separate energy reduction kernel instead of the fused final sweep")
     ap.add_argument("--cpu-steps", type=int, default=3, help="oracle steps timed for cpu_baseline")
     args = ap.parse_args()
     cfg = dict(hsg_inputs.CONFIGS[args.workload])

@@ -57,7 +57,11 @@ enum {
   HSG_KERNEL_ZMARCH = 2    /* one launch per hsg_sweep call: both colours of every sweep fused in a z-marching pass */
 };
 enum {
-  HSG_OPT_SWEEP_KERNEL = 1
+  HSG_OPT_SWEEP_KERNEL = 1,
+  HSG_OPT_FUSE_ENERGY = 2  /* 1 (default): the z-marching kernel reduces E and m of every system in the final
+                              sweep of each hsg_sweep call, so hsg_pt_swap / hsg_measure / hsg_energy right
+                              after it need no extra pass over the spins; 0: always use the separate
+                              reduction kernel.  Values agree to fp64 summation order (~1e-15 relative). */
 };
 
 typedef struct hsg_ctx hsg_ctx; /* opaque, host side */

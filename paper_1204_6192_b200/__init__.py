@@ -19,7 +19,7 @@ from . import _build
 
 HSG_OK, HSG_EINVAL, HSG_ESTATE, HSG_EUNSUPPORTED, HSG_ECUDA = 0, -1, -2, -3, -4
 HSG_KERNEL_AUTO, HSG_KERNEL_GENERIC, HSG_KERNEL_ZMARCH = 0, 1, 2
-HSG_OPT_SWEEP_KERNEL = 1
+HSG_OPT_SWEEP_KERNEL, HSG_OPT_FUSE_ENERGY = 1, 2
 KERNELS = {"auto": HSG_KERNEL_AUTO, "generic": HSG_KERNEL_GENERIC, "zmarch": HSG_KERNEL_ZMARCH}
 
 # every symbol include/hsg.h declares (tests check that the library exports each of them)

@@ -92,6 +92,7 @@ struct hsg_ctx {
   bool have_disorder, have_spins;
   bool energy_valid;            // e_slot / m_slot hold the reduction of the current spins
   int sweep_kernel_opt;
+  bool fuse_energy;             // zmarch: reduce E and m in the final sweep of every hsg_sweep call
   const char* last_kernel;
   unsigned long long launches;
   std::string err;
@@ -140,7 +141,7 @@ int hsg_create(const hsg_desc* desc, void* dev_state, size_t state_bytes, void* 
   c->e_slot = (double*)(s + sl.e_slot); c->m_slot = (double*)(s + sl.m_slot);
   c->e_partial = (double*)(w + cl.e_partial); c->q_partial = (double*)(w + cl.q_partial);
   c->k_hb = 0; c->k_pt = 0; c->have_disorder = false; c->have_spins = false; c->energy_valid = false;
-  c->sweep_kernel_opt = HSG_KERNEL_AUTO; c->last_kernel = "none"; c->launches = 0;
+  c->sweep_kernel_opt = HSG_KERNEL_AUTO; c->fuse_energy = true; c->last_kernel = "none"; c->launches = 0;
 
   // small host-computed tables: beta_t = (float)(1.0/(double)T_t); cos/sin(2 pi x / L) in fp64
   std::vector<float> beta(g.T);
@@ -178,6 +179,10 @@ int hsg_set_option(hsg_ctx* ctx, int option, int value) {
     if (value < HSG_KERNEL_AUTO || value > HSG_KERNEL_ZMARCH) HSG_FAIL(ctx, HSG_EINVAL, "unknown sweep kernel");
     if (value == HSG_KERNEL_ZMARCH && !zmarch_supported(ctx->g)) HSG_FAIL(ctx, HSG_EUNSUPPORTED, "zmarch kernel does not support this geometry");
     ctx->sweep_kernel_opt = value;
+    return HSG_OK;
+  }
+  if (option == HSG_OPT_FUSE_ENERGY) {
+    ctx->fuse_energy = value != 0;
     return HSG_OK;
   }
   HSG_FAIL(ctx, HSG_EINVAL, "unknown option");
@@ -248,13 +253,16 @@ int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
   int kernel = ctx->sweep_kernel_opt;
   if (kernel == HSG_KERNEL_AUTO) kernel = zmarch_supported(ctx->g) ? HSG_KERNEL_ZMARCH : HSG_KERNEL_GENERIC;
   if (kernel == HSG_KERNEL_ZMARCH) {
-    ZmarchArgs a{ctx->g, ctx->spins, ctx->jh, ctx->temp_of_slot, ctx->beta, ctx->key, ctx->k_hb, n_or, n_hb};
+    // the final sweep of the call also reduces E and m of every slot
+    ZmarchArgs a{ctx->g, ctx->spins, ctx->jh, ctx->temp_of_slot, ctx->beta, ctx->key, ctx->k_hb, n_or, n_hb,
+                 ctx->fuse_energy ? ctx->e_slot : nullptr, ctx->m_slot};
     int n_launch = 0;
     const cudaError_t e = zmarch_launch(a, ctx->stream, &n_launch);
     ctx->launches += (unsigned long long)n_launch;
     if (e != cudaSuccess) { ctx->err = std::string("zmarch launch: ") + cudaGetErrorString(e); return HSG_ECUDA; }
     ctx->k_hb += (unsigned long long)n_hb;
     ctx->last_kernel = "zmarch";
+    ctx->energy_valid = ctx->fuse_energy;
     return HSG_OK;
   }
   for (int s = 0; s < n_or; ++s) { const int rc = launch_generic_sweep(ctx, false); if (rc != HSG_OK) return rc; }

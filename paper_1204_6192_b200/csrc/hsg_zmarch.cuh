@@ -33,6 +33,8 @@ struct ZmarchArgs {
   PhiloxKey key;
   unsigned long long k_hb;      // heat-bath sweep counter of the first HB sweep of this call
   int n_or, n_hb;
+  double* e_slot;               // [R]    energy of every slot after the call, or nullptr
+  double* m_slot;               // [R][3] magnetisation of every slot after the call
 };
 
 namespace zm {
@@ -106,7 +108,10 @@ template <int L, int V, int G> struct Cfg {
   static constexpr int CS = L * Lh;               // one [y][j] array
   static constexpr int HP = 3 * CS;               // spin half-plane (one colour, 3 components)
   static constexpr int JP = 12 * CS;              // J/H plane (2 colours x 6 arrays)
-  static constexpr uint32_t ring_off = 64;        // byte offsets inside dynamic shared memory
+  static constexpr int RW = TPS < 32 ? TPS : 32;  // shuffle width of the per-system reduction
+  static constexpr int WPS = TPS / RW;            // partial sums per system after the shuffle stage
+  static constexpr uint32_t red_off = 64;         // byte offsets inside dynamic shared memory: [G][WPS][4] doubles
+  static constexpr uint32_t ring_off = 64 + 128 * ((G * WPS * 32 + 127) / 128);
   static constexpr uint32_t x_off = ring_off + 4u * kRing * JP;
   static constexpr size_t smem_bytes = x_off + sizeof(float) * ((size_t)G * 4 * HP);
   static_assert(Lh % V == 0, "row length must be a multiple of the vector width");
@@ -122,17 +127,24 @@ struct Th {
 
 struct HbPar { float beta; uint32_t sysid, c1, c3; PhiloxKey key; };
 
+// fp64 partial sums of one thread in the final sweep of a call:
+// e = sum_{i in colour 1} s_i.(sum_6 J_ij s_j) + sum_i H_i.s_i  (= -E), m = sum_i s_i; exact fp32 x fp32 products
+struct EAcc { double e, mx, my, mz; };
+
 // Local field of V sites of colour `cu` in plane zp, accumulated in the order H, x+, x-, y+, y-, z+, z-
 // (DESIGN.md §3.1), then the move.  `q` = the thread's own column of the other colour in this plane,
 // `xs` = shared-memory half-plane of the other colour in this plane (rows y+-1 and the x edge),
 // `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1,
 // `jo` = J/H arrays of colour cu in plane zp, `jx` = arrays of the other colour in plane zp,
 // `jzlo` = Jz array of the other colour in plane zp-1 (shared-memory ring; all 32-bit shared addresses).
-template <int L, int V, bool HB>
+// EN = 0: move only; 1: also accumulate H_i.s_i and s_i of the NEW spin (colour 0 in the final sweep);
+// 2: additionally s_i.(sum_6 J_ij s_j) with every bond of the site (colour 1 in the final sweep, when all its
+// neighbours already hold their final values).
+template <int L, int V, bool HB, int EN>
 __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&own)[3][V], const float (&q)[3][V],
                                              const float (&zlo)[3][V], const float (&zhi)[3][V], uint32_t xs,
                                              uint32_t jo, uint32_t jx, uint32_t jzlo,
-                                             const Th& th, int off, const HbPar& hp, uint32_t site0) {
+                                             const Th& th, int off, const HbPar& hp, uint32_t site0, EAcc& ea) {
   constexpr uint32_t CSB = 4u * L * (L / 2);
   const uint32_t edge = off ? th.edge1 : th.edge0;
   float Jxp[V], Jxm[V], Jyp[V], Jym[V], Jzp[V], Jzm[V];
@@ -150,6 +162,8 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
   lds<V>(Jym, jx + CSB + th.rowm);
   lds<V>(Jzm, jzlo + th.row);
   float h[3][V];
+  float Hs[3][V];
+  double hd[3][V];
   const uint32_t xs_p = xs + th.rowp, xs_m = xs + th.rowm, xs_e = xs + edge;
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
@@ -170,6 +184,16 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
       acc = __fmaf_rn(Jzp[e], zhi[mu][e], acc);
       acc = __fmaf_rn(Jzm[e], zlo[mu][e], acc);
       h[mu][e] = acc;
+      if (EN >= 1) Hs[mu][e] = Hm[e];
+      if (EN == 2) {
+        double d = (double)Jxp[e] * (double)sxp;
+        d = fma((double)Jxm[e], (double)sxm, d);
+        d = fma((double)Jyp[e], (double)yp[e], d);
+        d = fma((double)Jym[e], (double)ym[e], d);
+        d = fma((double)Jzp[e], (double)zhi[mu][e], d);
+        d = fma((double)Jzm[e], (double)zlo[mu][e], d);
+        hd[mu][e] = d;
+      }
     }
   }
 #pragma unroll
@@ -185,6 +209,18 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
       s = or_reflect(sv, hv);
     }
     out[0][e] = s.x; out[1][e] = s.y; out[2][e] = s.z;
+    if (EN >= 1) {
+      const double sx = (double)s.x, sy = (double)s.y, sz = (double)s.z;
+      double d = (double)Hs[0][e] * sx;
+      d = fma((double)Hs[1][e], sy, d);
+      d = fma((double)Hs[2][e], sz, d);
+      if (EN == 2) {
+        d = fma(hd[0][e], sx, d);
+        d = fma(hd[1][e], sy, d);
+        d = fma(hd[2][e], sz, d);
+      }
+      ea.e += d; ea.mx += sx; ea.my += sy; ea.mz += sz;
+    }
   }
 }
 
@@ -231,9 +267,9 @@ __device__ __forceinline__ void ring_advance(const Smem& sm, const float* __rest
 }
 
 // One full sweep (both colours, all planes) of the G systems of this CTA.
-template <int L, int V, int G, bool HB>
+template <int L, int V, int G, bool HB, bool EN>
 __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ S, const float* __restrict__ jh_d,
-                                            const Th& th, const HbPar& hp, int qbase, Stream& st) {
+                                            const Th& th, const HbPar& hp, int qbase, Stream& st, EAcc& ea) {
   using C = Cfg<L, V, G>;
   constexpr int CS = C::CS, HP = C::HP, JP = C::JP, PS = 2 * C::HP;
   constexpr uint32_t CSB = 4u * CS, HPB = 4u * HP, JPB = 4u * JP;
@@ -252,7 +288,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   }
   __syncthreads();
   // main steps: colour 0 of plane k, then colour 1 of plane k-1
-#pragma unroll kUnroll
+#pragma unroll (EN ? 1 : kUnroll)
   for (int k = 0; k < L; ++k) {
     const int nd = qbase + k + 1;                       // newest J/H stream index this step reads (plane k)
     ring_advance<L, JP>(sm, jh_d, st, nd);
@@ -278,7 +314,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     const uint32_t par = (uint32_t)(k & 1);
     {
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * k));
-      update_sites<L, V, HB>(R, O, B, A, Cc, sm.x1 + par * HPB, jk, jk + 6 * CSB, jk1 + 8 * CSB, th, off, hp, site0);
+      update_sites<L, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.x1 + par * HPB, jk, jk + 6 * CSB, jk1 + 8 * CSB, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) {
         stg<V>(Sr + k * PS + mu * CS, R[mu]);
@@ -288,7 +324,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     if (k >= 2) {     // colour 1 of plane k-1
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * (k - 1)));
       float N1[3][V];
-      update_sites<L, V, HB>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, jk1 + 6 * CSB, jk1, jk2 + 2 * CSB, th, off, hp, site0);
+      update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, jk1 + 6 * CSB, jk1, jk2 + 2 * CSB, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + (k - 1) * PS + HP + mu * CS, N1[mu]);
     }
@@ -326,7 +362,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     const int z1 = kk == 0 ? L - 1 : 0;
     const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * z1));
     float N1[3][V];
-    update_sites<L, V, HB>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, j1 + 6 * CSB, j1, j2 + 2 * CSB, th, off, hp, site0);
+    update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, j1 + 6 * CSB, j1, j2 + 2 * CSB, th, off, hp, site0, ea);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + z1 * PS + HP + mu * CS, N1[mu]);
     __syncthreads();
@@ -379,14 +415,41 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
   Stream st;
   st.issued = -1; st.waited = -1;
   st.total = n_sweeps * L + 2;                          // planes L-1, 0, 1, ..., L-1, 0, 1, ... (index q -> plane (q-1) mod L)
+  EAcc ea = {0.0, 0.0, 0.0, 0.0};
+  const bool want_e = a.e_slot != nullptr;
   for (int s = 0; s < n_sweeps; ++s) {
+    const bool fin = want_e && s + 1 == n_sweeps;       // the final sweep also reduces E and m
     if (s < a.n_or) {
       hp.c1 = 0; hp.c3 = 0;
-      march_sweep<L, V, G, false>(sm, S, jh_d, th, hp, s * L, st);
+      if (fin) march_sweep<L, V, G, false, true>(sm, S, jh_d, th, hp, s * L, st, ea);
+      else march_sweep<L, V, G, false, false>(sm, S, jh_d, th, hp, s * L, st, ea);
     } else {
       const unsigned long long khb = a.k_hb + (unsigned long long)(s - a.n_or);
       hp.c1 = (uint32_t)(khb & 0xFFFFFFFFull); hp.c3 = counter_hi(khb, DOMAIN_HB);
-      march_sweep<L, V, G, true>(sm, S, jh_d, th, hp, s * L, st);
+      if (fin) march_sweep<L, V, G, true, true>(sm, S, jh_d, th, hp, s * L, st, ea);
+      else march_sweep<L, V, G, true, false>(sm, S, jh_d, th, hp, s * L, st, ea);
+    }
+  }
+  if (want_e) {
+    // fixed-order reduction per system: lanes by shuffle, warps by one thread (deterministic)
+    constexpr int WPS = C::WPS, RW = C::RW;
+    double v[4] = {ea.e, ea.mx, ea.my, ea.mz};
+    double* red = reinterpret_cast<double*>(smem_raw + C::red_off);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+#pragma unroll
+      for (int o = RW / 2; o > 0; o >>= 1) v[i] += __shfl_down_sync(0xffffffffu, v[i], o, RW);
+    }
+    if (tl % RW == 0) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) red[(gs * WPS + tl / RW) * 4 + i] = v[i];
+    }
+    __syncthreads();
+    if (tl < 4) {
+      double x = 0.0;
+      for (int w = 0; w < WPS; ++w) x += red[(gs * WPS + w) * 4 + tl];
+      if (tl == 0) a.e_slot[slot] = -x;
+      else a.m_slot[slot * 3 + (tl - 1)] = x / (double)g.N;
     }
   }
 }

@@ -241,3 +241,27 @@ def test_branch_free_division_and_sqrt_are_ieee_correct():
     2e8 operand sets with random mantissas and exponents over [2^-100, 2^100]."""
     import paper_1204_6192_b200 as hsg
     assert hsg.hsg_selftest_arith(200_000_000, seed=12345) == (0, 0)
+
+
+@pytest.mark.parametrize("L,D,O,T", [(8, 1, 2, 16), (16, 2, 2, 4), (32, 1, 2, 4)])
+@pytest.mark.parametrize("n_or,n_hb", [(1, 0), (3, 0), (0, 1), (2, 2)])
+def test_energy_fused_into_the_last_sweep_matches_oracle_and_the_separate_reduction(L, D, O, T, n_or, n_hb):
+    """the z-marching kernel reduces E and m in the final sweep of a call (OR or HB)."""
+    import paper_1204_6192_b200 as hsg
+    eng, orc = _pair(L, D, O, T, seed=31, kernel="zmarch")
+    eng.init_spins(); orc.init_spins()
+    eng.sweep(n_or, n_hb); orc.sweep(n_or, n_hb)
+    n0 = eng.launch_count()
+    E, M, _, _ = (None if x is None else x.cpu().numpy() for x in eng.measure(out=(eng._new((D, O, T), eng.torch.float64),
+                                                                                 eng._new((D, O, T, 3), eng.torch.float64), None, None)))
+    assert eng.launch_count() - n0 == 2                  # two gathers, no reduction pass over the spins
+    Eo, Mo, _, _ = orc.measure()
+    np.testing.assert_allclose(E, Eo, rtol=1e-12)
+    np.testing.assert_allclose(M, Mo, rtol=0, atol=1e-13)
+    eng.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
+    eng.sweep(0, 0)                                      # no-op; cached values stay valid
+    eng2, _ = _pair(L, D, O, T, seed=31, kernel="zmarch")
+    eng2.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
+    eng2.init_spins(); eng2.sweep(n_or, n_hb)
+    np.testing.assert_allclose(eng2.energy().cpu().numpy(), E, rtol=1e-13)
+    assert np.array_equal(eng2.get_spins().cpu().numpy(), eng.get_spins().cpu().numpy())
