@@ -3,8 +3,8 @@
 // Checkerboard-compacted, plane-major SoA.  A site (x,y,z) has colour c = (x+y+z)&1 and compact
 // x-index j = x>>1, i.e. x = 2j + ((y+z+c)&1); Lh = L/2.
 //   spins of one configuration slot : S[z][c][mu][y][j]    fp32, 3N floats   (mu = spin component)
-//   disorder of one sample          : JH[z][c][k][y][j]    fp32, 6N floats   k=0,1,2: J of the bond
-//                                     from this site to +x,+y,+z ; k=3,4,5: H_x,H_y,H_z
+//   disorder of one sample          : JH[z][a][y][j]       fp32, 6N floats   a = jh_slot(c, k), k=0,1,2: J of
+//                                     the bond from this site to +x,+y,+z ; k=3,4,5: H_x,H_y,H_z
 // so that (i) all sites a colour update touches are unit-stride in j (128-bit vector loads, one
 // colour never interleaved with the other), (ii) the four y/z neighbours of compact site j sit at the
 // SAME j in the other colour's rows, the x neighbours at j and j-1 (or j+1), and (iii) one z-plane of
@@ -32,8 +32,14 @@ __host__ __device__ __forceinline__ long long jh_plane(const Geom& g) { return 1
 __host__ __device__ __forceinline__ long long spin_index(const Geom& g, int z, int c, int mu, int y, int j) {
   return (((long long)(z * 2 + c) * 3 + mu) * g.L + y) * g.Lh + j;
 }
+// Order of the twelve [y][j] arrays inside one J/H plane: everything a z-marching step needs for two steps
+// first (11 arrays, one bulk copy), the +z couplings of colour 0 last (needed for three steps, ring of its own):
+//   0,1: colour-0 Jx,Jy   2,3,4: colour-0 Hx,Hy,Hz   5,6,7: colour-1 Jx,Jy,Jz   8,9,10: colour-1 Hx,Hy,Hz   11: colour-0 Jz
+__host__ __device__ __forceinline__ int jh_slot(int c, int k) {
+  return c ? 5 + k : (k < 2 ? k : (k == 2 ? 11 : k - 1));
+}
 __host__ __device__ __forceinline__ long long jh_index(const Geom& g, int z, int c, int k, int y, int j) {
-  return (((long long)(z * 2 + c) * 6 + k) * g.L + y) * g.Lh + j;
+  return (((long long)z * 12 + jh_slot(c, k)) * g.L + y) * g.Lh + j;
 }
 
 }  // namespace hsg

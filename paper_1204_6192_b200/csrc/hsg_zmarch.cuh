@@ -8,15 +8,21 @@
 // deferred to the last step because it needs the new colour 0 of plane L-1).
 //
 //   * Thread ownership: thread (y, j0) of a system owns the V compact sites j0..j0+V-1 of row y in BOTH
-//     colours and in every plane.  All its global loads and stores go to its own column (128-bit,
-//     coalesced over the warp), so no inter-thread ordering of global memory is ever needed; the z
-//     neighbours of a site are the thread's own registers from the neighbouring steps.
-//   * In-plane neighbours (rows y-1, y+1 and the one x neighbour outside the thread's V sites) are
-//     exchanged through shared memory: X1 holds the old colour-1 spins of plane k, X0 the new colour-0
-//     spins of plane k-1, both double-buffered, one __syncthreads per step.
-//   * Couplings and fields of the sample stream through a 4-slot shared-memory ring filled by bulk
-//     async copies (cp.async.bulk, one 12*L*L/2-float plane per copy, mbarrier completion) issued one
-//     step ahead by thread 0, and are shared by the G systems of the CTA (PAPER.md:161's R_TO idea).
+//     colours and in every plane.  All its global loads and stores go to its own column, so no
+//     inter-thread ordering of global memory is ever needed; the z neighbours of a site are the thread's
+//     own registers from the neighbouring steps.
+//   * Spin planes are streamed global -> shared memory by per-thread cp.async copies of the thread's OWN
+//     column, DS steps ahead of their use (rings C1 = old colour-1 planes, C0 = old colour-0 planes).
+//     Completion is tracked per thread by cp.async groups, which (unlike register loads, whose scoreboard is
+//     shared with younger loads) lets a step wait for the oldest stage while DS-1 younger ones stay in
+//     flight: the bytes in flight per SM, not the issue rate, bound this kernel (Little's law).
+//   * In-plane neighbours (rows y-1, y+1 and the one x neighbour outside the thread's V sites) are read
+//     from shared memory: ring C1 holds the old colour-1 spins of plane k, X0 (double-buffered) the new
+//     colour-0 spins of plane k-1; one __syncthreads per step.
+//   * Couplings and fields of the sample stream through shared-memory rings filled by bulk async copies
+//     (cp.async.bulk, mbarrier completion) issued DJ steps ahead by thread 0, and are shared by the G
+//     systems of the CTA (PAPER.md:161's R_TO idea).  Eleven of the twelve arrays of a plane live for two
+//     steps (ring A); the +z couplings of colour 0 live for three (ring B).
 #pragma once
 #include <cuda_runtime.h>
 #include "hsg_layout.cuh"
@@ -43,22 +49,52 @@ namespace zm {
 #define HSG_ZM_UNROLL 2
 #endif
 #ifndef HSG_ZM_L32_V
-#define HSG_ZM_L32_V 2
+#define HSG_ZM_L32_V 4
 #endif
 #ifndef HSG_ZM_L32_G
 #define HSG_ZM_L32_G 2
 #endif
 #ifndef HSG_ZM_L16_V
-#define HSG_ZM_L16_V 2
+#define HSG_ZM_L16_V 4
 #endif
-constexpr int kRing = 4;
-constexpr int kUnroll = HSG_ZM_UNROLL;   // unroll factor of the main march loop   // J/H ring slots: planes k-2, k-1, k live + plane k+1 in flight
+#ifndef HSG_ZM_DS
+#define HSG_ZM_DS 2              // spin planes in flight ahead of the step that uses them
+#endif
+#ifndef HSG_ZM_DJ
+#define HSG_ZM_DJ 2              // J/H planes in flight ahead of the step that uses them
+#endif
+constexpr int kUnroll = HSG_ZM_UNROLL;   // unroll factor of the main march loop
+constexpr int kDS = HSG_ZM_DS, kDJ = HSG_ZM_DJ;
+constexpr int kNC1 = kDS + 2;            // ring C1: planes k, k+1 live + DS in flight
+constexpr int kNC0 = kDS + 1;            // ring C0: plane k live + DS in flight
+constexpr int kNJA = kDJ + 2;            // J/H ring A: planes k-1, k live + DJ in flight
+constexpr int kNJB = kDJ + 3;            // J/H ring B: planes k-2, k-1, k live + DJ in flight; also the mbarrier ring
 
-// ---------------------------------------------------------------- PTX wrappers: mbarrier + bulk async copy
+// ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+// per-thread async copy of 4V bytes global -> shared (streaming: evict-first in L2)
+template <int V> __device__ __forceinline__ void cp_async(uint32_t dst, const float* src, uint64_t pol);
+template <> __device__ __forceinline__ void cp_async<2>(uint32_t dst, const float* src, uint64_t pol) {
+  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "l"(pol) : "memory");
+}
+template <> __device__ __forceinline__ void cp_async<4>(uint32_t dst, const float* src, uint64_t pol) {
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ---------------------------------------------------------------- V-wide vector access (V = 2 or 4 floats)
 template <int V> struct VT;
@@ -107,15 +143,20 @@ template <int L, int V, int G> struct Cfg {
   static constexpr int NT = G * TPS;              // threads per CTA
   static constexpr int CS = L * Lh;               // one [y][j] array
   static constexpr int HP = 3 * CS;               // spin half-plane (one colour, 3 components)
-  static constexpr int JP = 12 * CS;              // J/H plane (2 colours x 6 arrays)
+  static constexpr int JP = 12 * CS;              // J/H plane: 11 arrays for ring A + colour-0 Jz for ring B
+  static constexpr int JA = 11 * CS;
   static constexpr int RW = TPS < 32 ? TPS : 32;  // shuffle width of the per-system reduction
   static constexpr int WPS = TPS / RW;            // partial sums per system after the shuffle stage
-  static constexpr uint32_t red_off = 64;         // byte offsets inside dynamic shared memory: [G][WPS][4] doubles
-  static constexpr uint32_t ring_off = 64 + 128 * ((G * WPS * 32 + 127) / 128);
-  static constexpr uint32_t x_off = ring_off + 4u * kRing * JP;
-  static constexpr size_t smem_bytes = x_off + sizeof(float) * ((size_t)G * 4 * HP);
+  // byte offsets inside dynamic shared memory
+  static constexpr uint32_t red_off = 64;         // [G][WPS][4] doubles (after kNJB <= 8 mbarriers)
+  static constexpr uint32_t ja_off = 64 + 128 * ((G * WPS * 32 + 127) / 128);
+  static constexpr uint32_t jb_off = ja_off + 4u * kNJA * JA;
+  static constexpr uint32_t sys_off = jb_off + 4u * kNJB * CS;
+  static constexpr uint32_t sys_bytes = 4u * (kNC1 + kNC0 + 2) * HP;     // per system: C1 ring, C0 ring, X0[2]
+  static constexpr size_t smem_bytes = sys_off + (size_t)G * sys_bytes;
   static_assert(Lh % V == 0, "row length must be a multiple of the vector width");
-  static_assert((JP * 4) % 16 == 0, "bulk copies move multiples of 16 bytes");
+  static_assert((CS * 4) % 16 == 0, "bulk copies move multiples of 16 bytes");
+  static_assert(kNJB <= 8, "mbarrier area holds 8 barriers");
 };
 
 // per-thread constants of the march (byte offsets inside a [y][j] array)
@@ -131,36 +172,41 @@ struct HbPar { float beta; uint32_t sysid, c1, c3; PhiloxKey key; };
 // e = sum_{i in colour 1} s_i.(sum_6 J_ij s_j) + sum_i H_i.s_i  (= -E), m = sum_i s_i; exact fp32 x fp32 products
 struct EAcc { double e, mx, my, mz; };
 
-// Local field of V sites of colour `cu` in plane zp, accumulated in the order H, x+, x-, y+, y-, z+, z-
+// shared-memory addresses of the coupling / field arrays one colour update reads
+struct JAddr {
+  uint32_t own_xy;   // own colour, this plane: Jx at +0, Jy at +CSB  (bonds to +x, +y)
+  uint32_t own_z;    // own colour, this plane: Jz                    (bond to +z)
+  uint32_t own_h;    // own colour, this plane: Hx, Hy, Hz at +0, +CSB, +2CSB
+  uint32_t oth_xy;   // other colour, this plane: Jx, Jy              (bonds from -x, -y)
+  uint32_t oth_z;    // other colour, plane below: Jz                 (bond from -z)
+};
+
+// Local field of V sites of one colour in plane zp, accumulated in the order H, x+, x-, y+, y-, z+, z-
 // (DESIGN.md §3.1), then the move.  `q` = the thread's own column of the other colour in this plane,
 // `xs` = shared-memory half-plane of the other colour in this plane (rows y+-1 and the x edge),
-// `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1,
-// `jo` = J/H arrays of colour cu in plane zp, `jx` = arrays of the other colour in plane zp,
-// `jzlo` = Jz array of the other colour in plane zp-1 (shared-memory ring; all 32-bit shared addresses).
+// `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1.
 // EN = 0: move only; 1: also accumulate H_i.s_i and s_i of the NEW spin (colour 0 in the final sweep);
 // 2: additionally s_i.(sum_6 J_ij s_j) with every bond of the site (colour 1 in the final sweep, when all its
 // neighbours already hold their final values).
 template <int L, int V, bool HB, int EN>
 __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&own)[3][V], const float (&q)[3][V],
                                              const float (&zlo)[3][V], const float (&zhi)[3][V], uint32_t xs,
-                                             uint32_t jo, uint32_t jx, uint32_t jzlo,
-                                             const Th& th, int off, const HbPar& hp, uint32_t site0, EAcc& ea) {
+                                             const JAddr& ja, const Th& th, int off, const HbPar& hp, uint32_t site0, EAcc& ea) {
   constexpr uint32_t CSB = 4u * L * (L / 2);
   const uint32_t edge = off ? th.edge1 : th.edge0;
   float Jxp[V], Jxm[V], Jyp[V], Jym[V], Jzp[V], Jzm[V];
-  const uint32_t jo_row = jo + th.row;
-  lds<V>(Jxp, jo_row);
-  lds<V>(Jyp, jo_row + CSB);
-  lds<V>(Jzp, jo_row + 2 * CSB);
+  lds<V>(Jxp, ja.own_xy + th.row);
+  lds<V>(Jyp, ja.own_xy + CSB + th.row);
+  lds<V>(Jzp, ja.own_z + th.row);
   {
     float t[V];
-    lds<V>(t, jx + th.row);
-    const float te = lds1(jx + th.edge0);
+    lds<V>(t, ja.oth_xy + th.row);
+    const float te = lds1(ja.oth_xy + th.edge0);
 #pragma unroll
     for (int e = 0; e < V; ++e) Jxm[e] = off ? t[e] : (e > 0 ? t[e > 0 ? e - 1 : 0] : te);
   }
-  lds<V>(Jym, jx + CSB + th.rowm);
-  lds<V>(Jzm, jzlo + th.row);
+  lds<V>(Jym, ja.oth_xy + CSB + th.rowm);
+  lds<V>(Jzm, ja.oth_z + th.row);
   float h[3][V];
   float Hs[3][V];
   double hd[3][V];
@@ -168,7 +214,7 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
     float Hm[V], yp[V], ym[V];
-    lds<V>(Hm, jo_row + (3 + mu) * CSB);
+    lds<V>(Hm, ja.own_h + mu * CSB + th.row);
     lds<V>(yp, xs_p + mu * CSB);
     lds<V>(ym, xs_m + mu * CSB);
     const float se = lds1(xs_e + mu * CSB);
@@ -226,34 +272,40 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
 
 // Shared state of one CTA during the march (32-bit shared-window addresses)
 struct Smem {
-  uint32_t full;       // [kRing] mbarriers
-  uint32_t ring;       // [kRing][JP] floats
+  uint32_t full;       // [kNJB] mbarriers
+  uint32_t ja, jb;     // J/H rings A ([kNJA][11 CS]) and B ([kNJB][CS])
+  uint32_t c1, c0;     // this thread's system: rings of old colour-1 / colour-0 half-planes
   uint32_t x0;         // this thread's system: [2][HP] new colour-0 spins of planes k-1, k
-  uint32_t x1;         // this thread's system: [2][HP] old colour-1 spins of planes k, k+1
 };
 
 struct Stream {        // J/H plane stream: index q -> plane (q-1) mod L
   int issued, waited, total;
 };
 
-template <int L, int JP>
-__device__ __forceinline__ void ring_advance(const Smem& sm, const float* __restrict__ jh_d, Stream& st, int nd) {
-  if (threadIdx.x == 0) {                               // producer: keep one plane in flight
-    const int upto = min(nd + 1, st.total - 1);
+// J/H stream: thread 0 keeps kDJ planes in flight beyond the newest index `nd` this step reads; everyone waits for nd.
+// Slot reuse is safe because the __syncthreads that ended the previous step separates the last reads of index
+// nd-2 (ring A) and nd-3 (ring B) from the copies issued here.
+template <int L, int CS>
+__device__ __forceinline__ void ring_advance(const Smem& sm, const float* __restrict__ jh_d, Stream& st, int nd, uint64_t pol) {
+  constexpr uint32_t JAB = 44u * CS, JBB = 4u * CS;
+  if (threadIdx.x == 0) {
+    const int upto = min(nd + kDJ, st.total - 1);
     while (st.issued < upto) {
       ++st.issued;
       const int plane = (st.issued + L - 1) % L;
-      const uint32_t slot = (uint32_t)st.issued % kRing;
-      const uint32_t bar = sm.full + 8u * slot;
-      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((uint32_t)JP * 4u) : "memory");
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                   ::"r"(sm.ring + slot * (uint32_t)JP * 4u), "l"(jh_d + (size_t)plane * JP), "r"((uint32_t)JP * 4u), "r"(bar) : "memory");
+      const uint32_t bar = sm.full + 8u * ((uint32_t)st.issued % kNJB);
+      const float* src = jh_d + (size_t)plane * 12 * CS;
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(JAB + JBB) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                   ::"r"(sm.ja + ((uint32_t)st.issued % kNJA) * JAB), "l"(src), "r"(JAB), "r"(bar), "l"(pol) : "memory");
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                   ::"r"(sm.jb + ((uint32_t)st.issued % kNJB) * JBB), "l"(src + 11 * CS), "r"(JBB), "r"(bar), "l"(pol) : "memory");
     }
   }
   while (st.waited < nd) {
     ++st.waited;
-    const uint32_t bar = sm.full + 8u * ((uint32_t)st.waited % kRing);
-    const uint32_t parity = ((uint32_t)st.waited / kRing) & 1u;
+    const uint32_t bar = sm.full + 8u * ((uint32_t)st.waited % kNJB);
+    const uint32_t parity = ((uint32_t)st.waited / kNJB) & 1u;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
@@ -269,52 +321,72 @@ __device__ __forceinline__ void ring_advance(const Smem& sm, const float* __rest
 // One full sweep (both colours, all planes) of the G systems of this CTA.
 template <int L, int V, int G, bool HB, bool EN>
 __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ S, const float* __restrict__ jh_d,
-                                            const Th& th, const HbPar& hp, int qbase, Stream& st, EAcc& ea) {
+                                            const Th& th, const HbPar& hp, int qbase, Stream& st, EAcc& ea,
+                                            uint64_t pol_spin, uint64_t pol_jh) {
   using C = Cfg<L, V, G>;
-  constexpr int CS = C::CS, HP = C::HP, JP = C::JP, PS = 2 * C::HP;
-  constexpr uint32_t CSB = 4u * CS, HPB = 4u * HP, JPB = 4u * JP;
-  float A[3][V], B[3][V], Cc[3][V], O[3][V], P[3][V], Q[3][V], R[3][V], Cn[3][V], On[3][V];
+  constexpr int CS = C::CS, HP = C::HP, PS = 2 * C::HP;
+  constexpr uint32_t CSB = 4u * CS, HPB = 4u * HP, JAB = 44u * CS, JBB = 4u * CS;
+  float A[3][V], B[3][V], Cc[3][V], O[3][V], P[3][V], Q[3][V], R[3][V], On[3][V];
   float* Sr = S + (th.row >> 2);                       // own column, plane 0, colour 0, component 0
-  // prologue: A = c1old(L-1), B = c1old(0) (published in X1[0]), prefetch c1old(1) and c0old(0)
+
+  // stage t = the planes step t consumes for the first time: old colour 1 of plane t+1 (ring C1, slot (t+1) % kNC1)
+  // and, for over-relaxation, old colour 0 of plane t (ring C0, slot t % kNC0); own column only.
+  auto issue_stage = [&](int t) {
+    if (t < L) {
+      const int zc = (t + 1 == L) ? 0 : t + 1;
+      const uint32_t d1 = sm.c1 + (uint32_t)((t + 1) % kNC1) * HPB + th.row;
+      const uint32_t d0 = sm.c0 + (uint32_t)(t % kNC0) * HPB + th.row;
+#pragma unroll
+      for (int mu = 0; mu < 3; ++mu) {
+        cp_async<V>(d1 + mu * CSB, Sr + zc * PS + HP + mu * CS, pol_spin);
+        if (!HB) cp_async<V>(d0 + mu * CSB, Sr + t * PS + mu * CS, pol_spin);
+      }
+    }
+    cp_async_commit();                                  // an empty group keeps the group count uniform
+  };
+
+  // prologue: B = c1old(0) through ring slot 0 (the whole plane is needed there), A = c1old(L-1), stages 0..DS-1
+#pragma unroll
+  for (int mu = 0; mu < 3; ++mu) cp_async<V>(sm.c1 + mu * CSB + th.row, Sr + HP + mu * CS, pol_spin);
+  cp_async_commit();
+#pragma unroll
+  for (int t = 0; t < kDS; ++t) issue_stage(t);
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
     ldg<V>(A[mu], Sr + (L - 1) * PS + HP + mu * CS);
-    ldg<V>(B[mu], Sr + HP + mu * CS);
-    ldg<V>(Cn[mu], Sr + 1 * PS + HP + mu * CS);
-    if (!HB) ldg<V>(On[mu], Sr + mu * CS);
 #pragma unroll
-    for (int e = 0; e < V; ++e) { P[mu][e] = 0.0f; Q[mu][e] = 0.0f; if (HB) On[mu][e] = 0.0f; }
-    sts<V>(sm.x1 + mu * CSB + th.row, B[mu]);
+    for (int e = 0; e < V; ++e) { P[mu][e] = 0.0f; Q[mu][e] = 0.0f; O[mu][e] = 0.0f; On[mu][e] = 0.0f; }
   }
+  cp_async_wait<kDS>();
+#pragma unroll
+  for (int mu = 0; mu < 3; ++mu) lds<V>(B[mu], sm.c1 + mu * CSB + th.row);
   __syncthreads();
   // main steps: colour 0 of plane k, then colour 1 of plane k-1
 #pragma unroll (EN ? 1 : kUnroll)
   for (int k = 0; k < L; ++k) {
     const int nd = qbase + k + 1;                       // newest J/H stream index this step reads (plane k)
-    ring_advance<L, JP>(sm, jh_d, st, nd);
+    ring_advance<L, CS>(sm, jh_d, st, nd, pol_jh);
+    cp_async_wait<kDS - 1>();                           // stage k has landed (own column)
 #pragma unroll
-    for (int mu = 0; mu < 3; ++mu)
-#pragma unroll
-      for (int e = 0; e < V; ++e) { Cc[mu][e] = Cn[mu][e]; O[mu][e] = On[mu][e]; }
-    if (k + 1 < L) {                                    // prefetch the next step's planes
-      const int zc = (k + 2 == L) ? 0 : k + 2;
-#pragma unroll
-      for (int mu = 0; mu < 3; ++mu) {
-        ldg<V>(Cn[mu], Sr + zc * PS + HP + mu * CS);
-        if (!HB) ldg<V>(On[mu], Sr + (k + 1) * PS + mu * CS);
-      }
-    } else {                                            // k = L-1: the new colour 0 of plane 0, needed by step L
+    for (int mu = 0; mu < 3; ++mu) {
+      lds<V>(Cc[mu], sm.c1 + (uint32_t)((k + 1) % kNC1) * HPB + mu * CSB + th.row);
+      if (!HB) lds<V>(O[mu], sm.c0 + (uint32_t)(k % kNC0) * HPB + mu * CSB + th.row);
+    }
+    issue_stage(k + kDS);
+    if (k + 1 == L) {                                   // the new colour 0 of plane 0, needed by step L
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) ldg<V>(On[mu], Sr + mu * CS);
     }
     const int off = (th.y + k) & 1;
-    const uint32_t jk = sm.ring + ((uint32_t)nd % kRing) * JPB;                  // plane k
-    const uint32_t jk1 = sm.ring + ((uint32_t)(nd + kRing - 1) % kRing) * JPB;   // plane k-1
-    const uint32_t jk2 = sm.ring + ((uint32_t)(nd + kRing - 2) % kRing) * JPB;   // plane k-2
+    const uint32_t ak = sm.ja + ((uint32_t)nd % kNJA) * JAB;                     // plane k
+    const uint32_t ak1 = sm.ja + ((uint32_t)(nd + kNJA - 1) % kNJA) * JAB;       // plane k-1
+    const uint32_t bk = sm.jb + ((uint32_t)nd % kNJB) * JBB;                     // colour-0 Jz of plane k
+    const uint32_t bk2 = sm.jb + ((uint32_t)(nd + kNJB - 2) % kNJB) * JBB;       // colour-0 Jz of plane k-2
     const uint32_t par = (uint32_t)(k & 1);
     {
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * k));
-      update_sites<L, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.x1 + par * HPB, jk, jk + 6 * CSB, jk1 + 8 * CSB, th, off, hp, site0, ea);
+      const JAddr ja = {ak, bk, ak + 2 * CSB, ak + 5 * CSB, ak1 + 7 * CSB};
+      update_sites<L, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % kNC1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) {
         stg<V>(Sr + k * PS + mu * CS, R[mu]);
@@ -323,14 +395,11 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     }
     if (k >= 2) {     // colour 1 of plane k-1
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * (k - 1)));
+      const JAddr ja = {ak1 + 5 * CSB, ak1 + 7 * CSB, ak1 + 8 * CSB, ak1, bk2};
       float N1[3][V];
-      update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, jk1 + 6 * CSB, jk1, jk2 + 2 * CSB, th, off, hp, site0, ea);
+      update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + (k - 1) * PS + HP + mu * CS, N1[mu]);
-    }
-    if (k + 1 < L) {
-#pragma unroll
-      for (int mu = 0; mu < 3; ++mu) sts<V>(sm.x1 + (par ^ 1u) * HPB + mu * CSB + th.row, Cc[mu]);
     }
     __syncthreads();
 #pragma unroll
@@ -338,13 +407,14 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
 #pragma unroll
       for (int e = 0; e < V; ++e) { A[mu][e] = B[mu][e]; B[mu][e] = Cc[mu][e]; P[mu][e] = Q[mu][e]; Q[mu][e] = R[mu][e]; }
   }
+  cp_async_wait<0>();                                   // only empty groups are left
   // tail: colour 1 of plane L-1 (step L) and of plane 0 (step L+1); their z+ neighbours are the new colour-0
   // spins of planes 0 and 1, read back from the thread's own column
 #pragma unroll 1
   for (int kk = 0; kk < 2; ++kk) {
     const int k = L + kk;
     const int nd = qbase + k;                            // plane k-1 (mod L)
-    ring_advance<L, JP>(sm, jh_d, st, nd);
+    ring_advance<L, CS>(sm, jh_d, st, nd, pol_jh);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
@@ -357,12 +427,13 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
       }
     }
     const int off = (th.y + k) & 1;
-    const uint32_t j1 = sm.ring + ((uint32_t)nd % kRing) * JPB;                  // plane k-1
-    const uint32_t j2 = sm.ring + ((uint32_t)(nd + kRing - 1) % kRing) * JPB;    // plane k-2
+    const uint32_t a1 = sm.ja + ((uint32_t)nd % kNJA) * JAB;                     // plane k-1
+    const uint32_t b2 = sm.jb + ((uint32_t)(nd + kNJB - 1) % kNJB) * JBB;        // colour-0 Jz of plane k-2
     const int z1 = kk == 0 ? L - 1 : 0;
     const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * z1));
+    const JAddr ja = {a1 + 5 * CSB, a1 + 7 * CSB, a1 + 8 * CSB, a1, b2};
     float N1[3][V];
-    update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, j1 + 6 * CSB, j1, j2 + 2 * CSB, th, off, hp, site0, ea);
+    update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + z1 * PS + HP + mu * CS, N1[mu]);
     __syncthreads();
@@ -381,12 +452,14 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
   const int gs = threadIdx.x / C::TPS, tl = threadIdx.x % C::TPS;
   Smem sm;
   sm.full = base;
-  sm.ring = base + C::ring_off;
-  sm.x0 = base + C::x_off + 4u * (uint32_t)(gs * 4) * C::HP;
-  sm.x1 = sm.x0 + 4u * 2 * C::HP;
+  sm.ja = base + C::ja_off;
+  sm.jb = base + C::jb_off;
+  sm.c1 = base + C::sys_off + (uint32_t)gs * C::sys_bytes;
+  sm.c0 = sm.c1 + 4u * kNC1 * C::HP;
+  sm.x0 = sm.c0 + 4u * kNC0 * C::HP;
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int i = 0; i < kRing; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    for (int i = 0; i < kNJB; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -410,6 +483,8 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
   hp.key = a.key;
   float* S = a.spins + (size_t)slot * 3 * g.N;
   const float* jh_d = a.jh + (size_t)d * 6 * g.N;
+  const uint64_t pol_spin = policy_evict_first();       // spins stream through L2 once per sweep
+  const uint64_t pol_jh = policy_evict_last();          // J/H of a sample are re-read by the CTAs of its O*T/G groups
 
   const int n_sweeps = a.n_or + a.n_hb;
   Stream st;
@@ -421,13 +496,13 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
     const bool fin = want_e && s + 1 == n_sweeps;       // the final sweep also reduces E and m
     if (s < a.n_or) {
       hp.c1 = 0; hp.c3 = 0;
-      if (fin) march_sweep<L, V, G, false, true>(sm, S, jh_d, th, hp, s * L, st, ea);
-      else march_sweep<L, V, G, false, false>(sm, S, jh_d, th, hp, s * L, st, ea);
+      if (fin) march_sweep<L, V, G, false, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
+      else march_sweep<L, V, G, false, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
     } else {
       const unsigned long long khb = a.k_hb + (unsigned long long)(s - a.n_or);
       hp.c1 = (uint32_t)(khb & 0xFFFFFFFFull); hp.c3 = counter_hi(khb, DOMAIN_HB);
-      if (fin) march_sweep<L, V, G, true, true>(sm, S, jh_d, th, hp, s * L, st, ea);
-      else march_sweep<L, V, G, true, false>(sm, S, jh_d, th, hp, s * L, st, ea);
+      if (fin) march_sweep<L, V, G, true, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
+      else march_sweep<L, V, G, true, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
     }
   }
   if (want_e) {
@@ -457,8 +532,6 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
 }  // namespace zm
 
 // ------------------------------------------------------------------------------------------------ host side
-struct ZmarchVariant { int L, V, G; };
-
 template <int L, int V, int G>
 inline cudaError_t zmarch_launch_t(const ZmarchArgs& a, cudaStream_t stream) {
   using C = zm::Cfg<L, V, G>;
