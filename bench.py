@@ -309,6 +309,8 @@ def main():
     ap.add_argument("--workload", default="c4", choices=sorted(hsg_inputs.CONFIGS))
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "zmarch"])
     ap.add_argument("--samples", type=int, default=None, help="override the number of disorder samples per GPU")
+    ap.add_argument("--n-or", type=int, default=None, help="override the over-relaxation sweeps per step (OR-only / HB-only timing points)")
+    ap.add_argument("--n-hb", type=int, default=None, help="override the heat-bath sweeps per step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-measure", action="store_true")
     ap.add_argument("--no-fuse-energy", action="store_true", help="separate energy reduction kernel instead of the fused final sweep")
@@ -317,6 +319,10 @@ def main():
     cfg = dict(hsg_inputs.CONFIGS[args.workload])
     if args.samples is not None:
         cfg["n_samples"] = args.samples
+    if args.n_or is not None:
+        cfg["n_or"] = args.n_or
+    if args.n_hb is not None:
+        cfg["n_hb"] = args.n_hb
     if cfg["t_min"] == cfg["t_max"]:
         temps = (cfg["t_min"] * (1.0 + 1e-6 * np.arange(cfg["n_temps"]))).astype(np.float32)
     else:

@@ -63,7 +63,11 @@ namespace zm {
 #ifndef HSG_ZM_DJ
 #define HSG_ZM_DJ 2              // J/H planes in flight ahead of the step that uses them
 #endif
+#ifndef HSG_ZM_UNROLL_HB
+#define HSG_ZM_UNROLL_HB 2
+#endif
 constexpr int kUnroll = HSG_ZM_UNROLL;   // unroll factor of the main march loop
+constexpr int kUnrollHB = HSG_ZM_UNROLL_HB;
 constexpr int kDS = HSG_ZM_DS, kDJ = HSG_ZM_DJ;
 constexpr int kNC1 = kDS + 2;            // ring C1: planes k, k+1 live + DS in flight
 constexpr int kNC0 = kDS + 1;            // ring C0: plane k live + DS in flight
@@ -362,7 +366,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   for (int mu = 0; mu < 3; ++mu) lds<V>(B[mu], sm.c1 + mu * CSB + th.row);
   __syncthreads();
   // main steps: colour 0 of plane k, then colour 1 of plane k-1
-#pragma unroll (EN ? 1 : kUnroll)
+#pragma unroll (EN ? 1 : (HB ? kUnrollHB : kUnroll))
   for (int k = 0; k < L; ++k) {
     const int nd = qbase + k + 1;                       // newest J/H stream index this step reads (plane k)
     ring_advance<L, CS>(sm, jh_d, st, nd, pol_jh);
@@ -566,13 +570,16 @@ inline cudaError_t zmarch_launch(const ZmarchArgs& a, cudaStream_t stream, int* 
 #if HSG_ZM_L32_G > 1
     HSG_ZM_CASE(32, HSG_ZM_L32_V, 1)
 #endif
-  } else if (a.g.L == 16) {
+  }
+#ifndef HSG_ZM_ONLY_L32     // (variant builds for experiments instantiate L = 32 only)
+  else if (a.g.L == 16) {
     const int G = zmarch_pick_g(a.g, 8);
     HSG_ZM_CASE(16, HSG_ZM_L16_V, 8) HSG_ZM_CASE(16, HSG_ZM_L16_V, 4) HSG_ZM_CASE(16, HSG_ZM_L16_V, 2) HSG_ZM_CASE(16, HSG_ZM_L16_V, 1)
   } else if (a.g.L == 8) {
     const int G = zmarch_pick_g(a.g, 8);
     HSG_ZM_CASE(8, 2, 8) HSG_ZM_CASE(8, 2, 4) HSG_ZM_CASE(8, 2, 2) HSG_ZM_CASE(8, 2, 1)
   }
+#endif
   *n_launch = 0;
   return cudaErrorNotSupported;
 }
