@@ -23,6 +23,12 @@
 //     (cp.async.bulk, mbarrier completion) issued DJ steps ahead by thread 0, and are shared by the G
 //     systems of the CTA (PAPER.md:161's R_TO idea).  Eleven of the twelve arrays of a plane live for two
 //     steps (ring A); the +z couplings of colour 0 live for three (ring B).
+//   * Lattices whose planes do not fit one SM's shared memory (L = 64) are split into L/YS strips of YS rows;
+//     the strips of a system group are the CTAs of one thread-block cluster.  Every shared array then carries
+//     halo rows: the old colour-1 halo rows are fetched from global memory by the edge threads (the owner
+//     overwrites them only two cluster barriers later), the new colour-0 halo rows are pushed into the
+//     neighbour CTA's shared memory (st.shared::cluster) by the thread that computed them, and the
+//     one-per-step __syncthreads becomes a cluster barrier (arrive.release / wait.acquire).
 #pragma once
 #include <cuda_runtime.h>
 #include "hsg_layout.cuh"
@@ -100,6 +106,24 @@ template <> __device__ __forceinline__ void cp_async<4>(uint32_t dst, const floa
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// thread-block cluster helpers (strips of one lattice, see the header comment)
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t cta_addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(cta_addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void st_cluster_f64(uint32_t addr, double v) {
+  asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
+
 // ---------------------------------------------------------------- V-wide vector access (V = 2 or 4 floats)
 template <int V> struct VT;
 template <> struct VT<2> { using type = float2; };
@@ -125,6 +149,31 @@ template <> __device__ __forceinline__ void sts<2>(uint32_t a, const float (&r)[
 template <> __device__ __forceinline__ void sts<4>(uint32_t a, const float (&r)[4]) {
   asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]) : "memory");
 }
+// asynchronous store into the shared memory of another CTA of the cluster (addresses from mapa_u32); the bytes are
+// counted on an mbarrier of THAT CTA, whose threads wait on it: no fence on either side
+template <int V> __device__ __forceinline__ void st_async(uint32_t a, const float (&r)[V], uint32_t bar);
+template <> __device__ __forceinline__ void st_async<2>(uint32_t a, const float (&r)[2], uint32_t bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1,%2}, [%3];"
+               ::"r"(a), "f"(r[0]), "f"(r[1]), "r"(bar) : "memory");
+}
+template <> __device__ __forceinline__ void st_async<4>(uint32_t a, const float (&r)[4], uint32_t bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1,%2,%3,%4}, [%5];"
+               ::"r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
 // streaming global access for the spins: each value is touched once per sweep
 template <int V> __device__ __forceinline__ void ldg(float (&r)[V], const float* p) {
   const typename VT<V>::type t = __ldcs(reinterpret_cast<const typename VT<V>::type*>(p));
@@ -140,34 +189,50 @@ template <int V> __device__ __forceinline__ void stg(float* p, const float (&r)[
   __stcs(reinterpret_cast<typename VT<V>::type*>(p), t);
 }
 
-template <int L, int V, int G> struct Cfg {
+template <int L, int YS, int V, int G> struct Cfg {
   static constexpr int Lh = L / 2;
+  static constexpr int YSv = YS;
+  static constexpr int NCL = L / YS;              // strips per lattice = CTAs per cluster
+  static constexpr bool HALO = NCL > 1;
   static constexpr int TPR = Lh / V;              // threads per row
-  static constexpr int TPS = L * TPR;             // threads per system
+  static constexpr int TPS = YS * TPR;            // threads per system (strip)
   static constexpr int NT = G * TPS;              // threads per CTA
-  static constexpr int CS = L * Lh;               // one [y][j] array
-  static constexpr int HP = 3 * CS;               // spin half-plane (one colour, 3 components)
-  static constexpr int JP = 12 * CS;              // J/H plane: 11 arrays for ring A + colour-0 Jz for ring B
-  static constexpr int JA = 11 * CS;
+  static constexpr int CSG = L * Lh;              // one [y][j] array in global memory
+  static constexpr int HPG = 3 * CSG;             // spin half-plane (one colour, 3 components) in global memory
+  static constexpr int CSS = (YS + (HALO ? 2 : 0)) * Lh;   // shared spin array: halo row below, YS rows, halo row above
+  static constexpr int HPS = 3 * CSS;
+  static constexpr int CSJ = (YS + (HALO ? 1 : 0)) * Lh;   // shared J/H array: halo row below (for the -y couplings), YS rows
+  static constexpr int JA = 11 * CSJ;             // ring A slot: 11 arrays; ring B slot: colour-0 Jz
   static constexpr int RW = TPS < 32 ? TPS : 32;  // shuffle width of the per-system reduction
   static constexpr int WPS = TPS / RW;            // partial sums per system after the shuffle stage
   // byte offsets inside dynamic shared memory
-  static constexpr uint32_t red_off = 64;         // [G][WPS][4] doubles (after kNJB <= 8 mbarriers)
-  static constexpr uint32_t ja_off = 64 + 128 * ((G * WPS * 32 + 127) / 128);
+  static constexpr uint32_t red_off = 64;         // [G][WPS][4] doubles (after kNJB <= 6 J/H mbarriers and 2 halo mbarriers)
+  static constexpr uint32_t red2_off = red_off + G * WPS * 32;        // [G][NCL][4] doubles: per-strip sums, used in rank 0
+  static constexpr uint32_t ja_off = 128 * ((red2_off + G * NCL * 32 + 127) / 128);
   static constexpr uint32_t jb_off = ja_off + 4u * kNJA * JA;
-  static constexpr uint32_t sys_off = jb_off + 4u * kNJB * CS;
-  static constexpr uint32_t sys_bytes = 4u * (kNC1 + kNC0 + 2) * HP;     // per system: C1 ring, C0 ring, X0[2]
+  static constexpr uint32_t sys_off = jb_off + 4u * kNJB * CSJ;
+  static constexpr uint32_t sys_bytes = 4u * (kNC1 + kNC0 + 2) * HPS;    // per system: C1 ring, C0 ring, X0[2]
   static constexpr size_t smem_bytes = sys_off + (size_t)G * sys_bytes;
-  static_assert(Lh % V == 0, "row length must be a multiple of the vector width");
-  static_assert((CS * 4) % 16 == 0, "bulk copies move multiples of 16 bytes");
-  static_assert(kNJB <= 8, "mbarrier area holds 8 barriers");
+  static_assert(L % YS == 0 && Lh % V == 0, "strip height divides L, vector width divides the row length");
+  static_assert((YS * Lh * 4) % 16 == 0 && (Lh * 4) % 16 == 0, "bulk copies move multiples of 16 bytes");
+  static_assert(!HALO || V == 4, "halo copies use 16-byte cp.async.cg");
+  static_assert(!HALO || YS >= 2, "a thread is on at most one strip edge");
+  static_assert(kNJB <= 6, "mbarrier area holds kNJB J/H barriers and two halo barriers");
+  static constexpr uint32_t halo_bytes = G * 2u * 3u * Lh * 4u;   // new colour-0 halo rows received per step: both neighbours, G systems
+  static_assert(smem_bytes <= 232448, "exceeds the 227 KB of shared memory per CTA");
 };
 
-// per-thread constants of the march (byte offsets inside a [y][j] array)
+// per-thread constants of the march
 struct Th {
-  int y, j0;
-  uint32_t row, rowp, rowm;   // own row, row y+1, row y-1 (periodic) at j0
+  int gy, j0;                 // global row, first compact site
+  int grow;                   // gy * Lh + j0: element offset of the own column inside a global [y][j] array
+  int grow_halo;              // HALO edge threads: element offset of the halo row they fetch (row gy-1 or gy+1, periodic)
+  int edge;                   // HALO: -1 = lowest row of the strip, +1 = highest row, 0 = interior
+  uint32_t row, rowp, rowm;   // byte offsets inside a shared [y][j] array: own row, row y+1, row y-1 at j0
   uint32_t edge0, edge1;      // own row at j0-1 and j0+V (periodic): the x neighbour outside the thread's V sites
+  uint32_t halo;              // HALO edge threads: byte offset of the halo row they fill (== rowm or rowp)
+  uint32_t push;              // HALO edge threads: cluster address of X0[0], component 0, halo row at j0 in the neighbour CTA
+  uint32_t push_bar;          // HALO edge threads: cluster address of the neighbour CTA's halo mbarrier of X0[0]
 };
 
 struct HbPar { float beta; uint32_t sysid, c1, c3; PhiloxKey key; };
@@ -178,9 +243,9 @@ struct EAcc { double e, mx, my, mz; };
 
 // shared-memory addresses of the coupling / field arrays one colour update reads
 struct JAddr {
-  uint32_t own_xy;   // own colour, this plane: Jx at +0, Jy at +CSB  (bonds to +x, +y)
+  uint32_t own_xy;   // own colour, this plane: Jx at +0, Jy at +CJB  (bonds to +x, +y)
   uint32_t own_z;    // own colour, this plane: Jz                    (bond to +z)
-  uint32_t own_h;    // own colour, this plane: Hx, Hy, Hz at +0, +CSB, +2CSB
+  uint32_t own_h;    // own colour, this plane: Hx, Hy, Hz at +0, +CJB, +2CJB
   uint32_t oth_xy;   // other colour, this plane: Jx, Jy              (bonds from -x, -y)
   uint32_t oth_z;    // other colour, plane below: Jz                 (bond from -z)
 };
@@ -188,19 +253,19 @@ struct JAddr {
 // Local field of V sites of one colour in plane zp, accumulated in the order H, x+, x-, y+, y-, z+, z-
 // (DESIGN.md §3.1), then the move.  `q` = the thread's own column of the other colour in this plane,
 // `xs` = shared-memory half-plane of the other colour in this plane (rows y+-1 and the x edge),
-// `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1.
+// `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1.  CSB / CJB = byte strides between the
+// component arrays of a shared spin half-plane / between the arrays of a shared J/H plane.
 // EN = 0: move only; 1: also accumulate H_i.s_i and s_i of the NEW spin (colour 0 in the final sweep);
 // 2: additionally s_i.(sum_6 J_ij s_j) with every bond of the site (colour 1 in the final sweep, when all its
 // neighbours already hold their final values).
-template <int L, int V, bool HB, int EN>
+template <uint32_t CSB, uint32_t CJB, int V, bool HB, int EN>
 __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&own)[3][V], const float (&q)[3][V],
                                              const float (&zlo)[3][V], const float (&zhi)[3][V], uint32_t xs,
                                              const JAddr& ja, const Th& th, int off, const HbPar& hp, uint32_t site0, EAcc& ea) {
-  constexpr uint32_t CSB = 4u * L * (L / 2);
   const uint32_t edge = off ? th.edge1 : th.edge0;
   float Jxp[V], Jxm[V], Jyp[V], Jym[V], Jzp[V], Jzm[V];
   lds<V>(Jxp, ja.own_xy + th.row);
-  lds<V>(Jyp, ja.own_xy + CSB + th.row);
+  lds<V>(Jyp, ja.own_xy + CJB + th.row);
   lds<V>(Jzp, ja.own_z + th.row);
   {
     float t[V];
@@ -209,7 +274,7 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
 #pragma unroll
     for (int e = 0; e < V; ++e) Jxm[e] = off ? t[e] : (e > 0 ? t[e > 0 ? e - 1 : 0] : te);
   }
-  lds<V>(Jym, ja.oth_xy + CSB + th.rowm);
+  lds<V>(Jym, ja.oth_xy + CJB + th.rowm);
   lds<V>(Jzm, ja.oth_z + th.row);
   float h[3][V];
   float Hs[3][V];
@@ -218,7 +283,7 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
     float Hm[V], yp[V], ym[V];
-    lds<V>(Hm, ja.own_h + mu * CSB + th.row);
+    lds<V>(Hm, ja.own_h + mu * CJB + th.row);
     lds<V>(yp, xs_p + mu * CSB);
     lds<V>(ym, xs_m + mu * CSB);
     const float se = lds1(xs_e + mu * CSB);
@@ -276,34 +341,57 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
 
 // Shared state of one CTA during the march (32-bit shared-window addresses)
 struct Smem {
-  uint32_t full;       // [kNJB] mbarriers
-  uint32_t ja, jb;     // J/H rings A ([kNJA][11 CS]) and B ([kNJB][CS])
+  uint32_t full;       // [kNJB] mbarriers of the J/H stream
+  uint32_t hfull;      // [2] mbarriers: halo rows of X0[0], X0[1] have arrived from the neighbour strips
+  uint32_t ja, jb;     // J/H rings A ([kNJA][11 CSJ]) and B ([kNJB][CSJ])
   uint32_t c1, c0;     // this thread's system: rings of old colour-1 / colour-0 half-planes
-  uint32_t x0;         // this thread's system: [2][HP] new colour-0 spins of planes k-1, k
+  uint32_t x0;         // this thread's system: [2][HPS] new colour-0 spins of planes k-1, k
+  int y0;              // first row of this CTA's strip
 };
 
 struct Stream {        // J/H plane stream: index q -> plane (q-1) mod L
   int issued, waited, total;
 };
 
-// J/H stream: thread 0 keeps kDJ planes in flight beyond the newest index `nd` this step reads; everyone waits for nd.
-// Slot reuse is safe because the __syncthreads that ended the previous step separates the last reads of index
-// nd-2 (ring A) and nd-3 (ring B) from the copies issued here.
-template <int L, int CS>
+// J/H stream: warp 0 keeps kDJ planes in flight beyond the newest index `nd` this step reads; everyone waits for nd.
+// Slot reuse is safe because the barrier that ended the previous step separates the last reads of index
+// nd-2 (ring A) and nd-3 (ring B) from the copies issued here.  Whole-plane CTAs move a plane with two bulk copies;
+// strip CTAs move the YS rows of each of the twelve arrays plus the halo row of the two Jy arrays (14 copies, one per lane).
+template <class C, int L>
 __device__ __forceinline__ void ring_advance(const Smem& sm, const float* __restrict__ jh_d, Stream& st, int nd, uint64_t pol) {
-  constexpr uint32_t JAB = 44u * CS, JBB = 4u * CS;
-  if (threadIdx.x == 0) {
+  constexpr uint32_t JAB = 4u * C::JA, JBB = 4u * C::CSJ;
+  if (threadIdx.x < 32) {
     const int upto = min(nd + kDJ, st.total - 1);
     while (st.issued < upto) {
       ++st.issued;
       const int plane = (st.issued + L - 1) % L;
       const uint32_t bar = sm.full + 8u * ((uint32_t)st.issued % kNJB);
-      const float* src = jh_d + (size_t)plane * 12 * CS;
-      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(JAB + JBB) : "memory");
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                   ::"r"(sm.ja + ((uint32_t)st.issued % kNJA) * JAB), "l"(src), "r"(JAB), "r"(bar), "l"(pol) : "memory");
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                   ::"r"(sm.jb + ((uint32_t)st.issued % kNJB) * JBB), "l"(src + 11 * CS), "r"(JBB), "r"(bar), "l"(pol) : "memory");
+      const uint32_t dA = sm.ja + ((uint32_t)st.issued % kNJA) * JAB, dB = sm.jb + ((uint32_t)st.issued % kNJB) * JBB;
+      const float* src = jh_d + (size_t)plane * 12 * C::CSG;
+      if (!C::HALO) {
+        if (threadIdx.x == 0) {
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(JAB + JBB) : "memory");
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                       ::"r"(dA), "l"(src), "r"(JAB), "r"(bar), "l"(pol) : "memory");
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                       ::"r"(dB), "l"(src + 11 * C::CSG), "r"(JBB), "r"(bar), "l"(pol) : "memory");
+        }
+      } else {
+        constexpr uint32_t ROWB = 4u * C::Lh, STRIPB = 4u * C::YSv * C::Lh;
+        const int lane = (int)threadIdx.x;
+        if (lane == 0)
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(12u * STRIPB + 2u * ROWB) : "memory");
+        __syncwarp();
+        if (lane < 14) {
+          const int arr = lane < 12 ? lane : (lane == 12 ? 1 : 6);           // halo rows: colour-0 Jy, colour-1 Jy
+          const uint32_t dbase = arr < 11 ? dA + (uint32_t)arr * JBB : dB;
+          const uint32_t dst = lane < 12 ? dbase + ROWB : dbase;
+          const int srow = lane < 12 ? sm.y0 : (sm.y0 + L - 1) % L;
+          const uint32_t bytes = lane < 12 ? STRIPB : ROWB;
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                       ::"r"(dst), "l"(src + (size_t)arr * C::CSG + (size_t)srow * C::Lh), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+        }
+      }
     }
   }
   while (st.waited < nd) {
@@ -322,36 +410,80 @@ __device__ __forceinline__ void ring_advance(const Smem& sm, const float* __rest
   }
 }
 
+// The barrier that ends a step.  Inside the CTA it is a __syncthreads.  Between the strips of a cluster it is split:
+// every thread ARRIVES at the end of step j and WAITS in step j+1 just before it publishes its new colour-0 spins, so a
+// CTA runs up to half a step ahead of its neighbours.  What the cluster phase orders:
+//   * my colour-1 reads of the halo X0[(j-1)&1] in step j (before my arrive) -> the neighbour's push into the same
+//     buffer in step j+1 (after its wait);
+//   * my fetch of an old colour-1 halo row (waited for at the top of step z-1) -> the owner's store of the new row in step z+1.
+// Both are read-before-overwrite orders, so the per-step arrive is RELAXED (a releasing arrive would stall every step
+// until the step's global stores are acknowledged).  The pushed halo rows themselves are ordered by their mbarrier
+// (st.async complete_tx).  Only the last arrive of a sweep RELEASES, pairing with the acquiring wait of the next
+// prologue: it makes the new colour-1 rows in global memory visible to the neighbour that fetches them as halo rows.
+template <class C, bool RELEASE = false> __device__ __forceinline__ void step_end() {
+  __syncthreads();
+  if (C::HALO) { if (RELEASE) cluster_arrive(); else cluster_arrive_relaxed(); }
+}
+template <class C> __device__ __forceinline__ void step_wait() {
+  if (C::HALO) cluster_wait();
+}
+
 // One full sweep (both colours, all planes) of the G systems of this CTA.
-template <int L, int V, int G, bool HB, bool EN>
+template <int L, int YS, int V, int G, bool HB, bool EN>
 __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ S, const float* __restrict__ jh_d,
                                             const Th& th, const HbPar& hp, int qbase, Stream& st, EAcc& ea,
-                                            uint64_t pol_spin, uint64_t pol_jh) {
-  using C = Cfg<L, V, G>;
-  constexpr int CS = C::CS, HP = C::HP, PS = 2 * C::HP;
-  constexpr uint32_t CSB = 4u * CS, HPB = 4u * HP, JAB = 44u * CS, JBB = 4u * CS;
+                                            uint64_t pol_spin, uint64_t pol_jh, uint32_t& hph) {
+  using C = Cfg<L, YS, V, G>;
+  constexpr int CS = C::CSG, HP = C::HPG, PS = 2 * C::HPG;
+  constexpr uint32_t CSB = 4u * C::CSS, HPB = 4u * C::HPS, CJB = 4u * C::CSJ, JAB = 4u * C::JA, JBB = 4u * C::CSJ;
+  constexpr bool HALO = C::HALO;
   float A[3][V], B[3][V], Cc[3][V], O[3][V], P[3][V], Q[3][V], R[3][V], On[3][V];
-  float* Sr = S + (th.row >> 2);                       // own column, plane 0, colour 0, component 0
+  float* Sr = S + th.grow;                             // own column, plane 0, colour 0, component 0
+  const float* Sh = S + th.grow_halo;                  // HALO edge threads: the halo row they fetch
 
+  // old colour 1 of plane zc -> ring C1 slot `slot`: own column, plus the halo row of the strip's edge threads
+  auto fetch_c1 = [&](int zc, int slot) {
+    const uint32_t d1 = sm.c1 + (uint32_t)slot * HPB;
+#pragma unroll
+    for (int mu = 0; mu < 3; ++mu) {
+      cp_async<V>(d1 + mu * CSB + th.row, Sr + zc * PS + HP + mu * CS, pol_spin);
+      if (HALO && th.edge != 0) cp_async<V>(d1 + mu * CSB + th.halo, Sh + zc * PS + HP + mu * CS, pol_spin);
+    }
+  };
   // stage t = the planes step t consumes for the first time: old colour 1 of plane t+1 (ring C1, slot (t+1) % kNC1)
   // and, for over-relaxation, old colour 0 of plane t (ring C0, slot t % kNC0); own column only.
   auto issue_stage = [&](int t) {
     if (t < L) {
-      const int zc = (t + 1 == L) ? 0 : t + 1;
-      const uint32_t d1 = sm.c1 + (uint32_t)((t + 1) % kNC1) * HPB + th.row;
-      const uint32_t d0 = sm.c0 + (uint32_t)(t % kNC0) * HPB + th.row;
+      fetch_c1((t + 1 == L) ? 0 : t + 1, (t + 1) % kNC1);
+      if (!HB) {
+        const uint32_t d0 = sm.c0 + (uint32_t)(t % kNC0) * HPB + th.row;
 #pragma unroll
-      for (int mu = 0; mu < 3; ++mu) {
-        cp_async<V>(d1 + mu * CSB, Sr + zc * PS + HP + mu * CS, pol_spin);
-        if (!HB) cp_async<V>(d0 + mu * CSB, Sr + t * PS + mu * CS, pol_spin);
+        for (int mu = 0; mu < 3; ++mu) cp_async<V>(d0 + mu * CSB, Sr + t * PS + mu * CS, pol_spin);
       }
     }
     cp_async_commit();                                  // an empty group keeps the group count uniform
   };
+  // new colour-0 spins of a plane -> X0[par] of this CTA and, from the strip's edge rows, the neighbour CTA's halo row
+  auto publish_x0 = [&](uint32_t par, const float (&v)[3][V]) {
+#pragma unroll
+    for (int mu = 0; mu < 3; ++mu) {
+      sts<V>(sm.x0 + par * HPB + mu * CSB + th.row, v[mu]);
+      if (HALO && th.edge != 0) st_async<V>(th.push + par * HPB + mu * CSB, v[mu], th.push_bar + 8u * par);
+    }
+  };
+  // halo rows of X0[par]: thread 0 arms the mbarrier before the neighbours may push (they wait for this CTA's arrive of
+  // the previous step), every thread waits for the bytes before the colour-1 update that reads them; bit `par` of hph
+  // is the parity of the phase in flight
+  auto arm_halo = [&](uint32_t par) {
+    if (HALO && threadIdx.x == 0) mbar_expect_tx(sm.hfull + 8u * par, C::halo_bytes);
+  };
+  auto wait_halo = [&](uint32_t par) {
+    if (HALO) { mbar_wait(sm.hfull + 8u * par, (hph >> par) & 1u); hph ^= 1u << par; }
+  };
 
   // prologue: B = c1old(0) through ring slot 0 (the whole plane is needed there), A = c1old(L-1), stages 0..DS-1
-#pragma unroll
-  for (int mu = 0; mu < 3; ++mu) cp_async<V>(sm.c1 + mu * CSB + th.row, Sr + HP + mu * CS, pol_spin);
+  step_wait<C>();                                       // strips: the neighbours' stores of the previous sweep are visible
+  fetch_c1(0, 0);
   cp_async_commit();
 #pragma unroll
   for (int t = 0; t < kDS; ++t) issue_stage(t);
@@ -364,12 +496,13 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   cp_async_wait<kDS>();
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) lds<V>(B[mu], sm.c1 + mu * CSB + th.row);
-  __syncthreads();
+  step_end<C>();
   // main steps: colour 0 of plane k, then colour 1 of plane k-1
 #pragma unroll (EN ? 1 : (HB ? kUnrollHB : kUnroll))
   for (int k = 0; k < L; ++k) {
     const int nd = qbase + k + 1;                       // newest J/H stream index this step reads (plane k)
-    ring_advance<L, CS>(sm, jh_d, st, nd, pol_jh);
+    ring_advance<C, L>(sm, jh_d, st, nd, pol_jh);
+    arm_halo((uint32_t)(k & 1));
     cp_async_wait<kDS - 1>();                           // stage k has landed (own column)
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) {
@@ -381,31 +514,31 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) ldg<V>(On[mu], Sr + mu * CS);
     }
-    const int off = (th.y + k) & 1;
+    const int off = (th.gy + k) & 1;
     const uint32_t ak = sm.ja + ((uint32_t)nd % kNJA) * JAB;                     // plane k
     const uint32_t ak1 = sm.ja + ((uint32_t)(nd + kNJA - 1) % kNJA) * JAB;       // plane k-1
     const uint32_t bk = sm.jb + ((uint32_t)nd % kNJB) * JBB;                     // colour-0 Jz of plane k
     const uint32_t bk2 = sm.jb + ((uint32_t)(nd + kNJB - 2) % kNJB) * JBB;       // colour-0 Jz of plane k-2
     const uint32_t par = (uint32_t)(k & 1);
     {
-      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * k));
-      const JAddr ja = {ak, bk, ak + 2 * CSB, ak + 5 * CSB, ak1 + 7 * CSB};
-      update_sites<L, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % kNC1) * HPB, ja, th, off, hp, site0, ea);
+      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * k));
+      const JAddr ja = {ak, bk, ak + 2 * CJB, ak + 5 * CJB, ak1 + 7 * CJB};
+      update_sites<CSB, CJB, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % kNC1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
-      for (int mu = 0; mu < 3; ++mu) {
-        stg<V>(Sr + k * PS + mu * CS, R[mu]);
-        sts<V>(sm.x0 + par * HPB + mu * CSB + th.row, R[mu]);
-      }
+      for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + k * PS + mu * CS, R[mu]);
+      step_wait<C>();
+      publish_x0(par, R);
     }
+    if (k >= 1) wait_halo(par ^ 1u);                   // (step 0's rows are pushed again in the tail: consumed unread)
     if (k >= 2) {     // colour 1 of plane k-1
-      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * (k - 1)));
-      const JAddr ja = {ak1 + 5 * CSB, ak1 + 7 * CSB, ak1 + 8 * CSB, ak1, bk2};
+      const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * (k - 1)));
+      const JAddr ja = {ak1 + 5 * CJB, ak1 + 7 * CJB, ak1 + 8 * CJB, ak1, bk2};
       float N1[3][V];
-      update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, ja, th, off, hp, site0, ea);
+      update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + (k - 1) * PS + HP + mu * CS, N1[mu]);
     }
-    __syncthreads();
+    step_end<C>();
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
@@ -418,29 +551,31 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   for (int kk = 0; kk < 2; ++kk) {
     const int k = L + kk;
     const int nd = qbase + k;                            // plane k-1 (mod L)
-    ring_advance<L, CS>(sm, jh_d, st, nd, pol_jh);
+    ring_advance<C, L>(sm, jh_d, st, nd, pol_jh);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
       for (int e = 0; e < V; ++e) R[mu][e] = On[mu][e];
+    if (kk == 0) arm_halo(0u);
+    step_wait<C>();
     if (kk == 0) {
 #pragma unroll
-      for (int mu = 0; mu < 3; ++mu) {
-        ldg<V>(On[mu], Sr + PS + mu * CS);               // new colour 0 of plane 1, needed by step L+1
-        sts<V>(sm.x0 + mu * CSB + th.row, R[mu]);         // L is even: X0[L & 1] = X0[0] <- new colour 0 of plane 0
-      }
+      for (int mu = 0; mu < 3; ++mu) ldg<V>(On[mu], Sr + PS + mu * CS);   // new colour 0 of plane 1, needed by step L+1
+      publish_x0(0u, R);                                 // L is even: X0[L & 1] = X0[0] <- new colour 0 of plane 0
     }
-    const int off = (th.y + k) & 1;
+    wait_halo((uint32_t)((k - 1) & 1));
+    const int off = (th.gy + k) & 1;
     const uint32_t a1 = sm.ja + ((uint32_t)nd % kNJA) * JAB;                     // plane k-1
     const uint32_t b2 = sm.jb + ((uint32_t)(nd + kNJB - 1) % kNJB) * JBB;        // colour-0 Jz of plane k-2
     const int z1 = kk == 0 ? L - 1 : 0;
-    const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.y + L * z1));
-    const JAddr ja = {a1 + 5 * CSB, a1 + 7 * CSB, a1 + 8 * CSB, a1, b2};
+    const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * z1));
+    const JAddr ja = {a1 + 5 * CJB, a1 + 7 * CJB, a1 + 8 * CJB, a1, b2};
     float N1[3][V];
-    update_sites<L, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, ja, th, off, hp, site0, ea);
+    update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + z1 * PS + HP + mu * CS, N1[mu]);
-    __syncthreads();
+    if (kk == 1) step_end<C, true>();
+    else step_end<C>();
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
@@ -448,36 +583,61 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   }
 }
 
-template <int L, int V, int G>
-__global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs a) {
-  using C = Cfg<L, V, G>;
+template <int L, int YS, int V, int G>
+__global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchArgs a) {
+  using C = Cfg<L, YS, V, G>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const uint32_t base = smem_u32(smem_raw);
   const int gs = threadIdx.x / C::TPS, tl = threadIdx.x % C::TPS;
+  const int rank = C::HALO ? (int)cluster_ctarank() : 0;   // strip index
+  const int group = C::HALO ? (int)(blockIdx.x / C::NCL) : (int)blockIdx.x;
   Smem sm;
   sm.full = base;
+  sm.hfull = base + 48;
   sm.ja = base + C::ja_off;
   sm.jb = base + C::jb_off;
   sm.c1 = base + C::sys_off + (uint32_t)gs * C::sys_bytes;
-  sm.c0 = sm.c1 + 4u * kNC1 * C::HP;
-  sm.x0 = sm.c0 + 4u * kNC0 * C::HP;
+  sm.c0 = sm.c1 + 4u * kNC1 * C::HPS;
+  sm.x0 = sm.c0 + 4u * kNC0 * C::HPS;
+  sm.y0 = rank * YS;
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int i = 0; i < kNJB; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + 6, 1);
+    mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + 7, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncthreads();
+  step_end<C, true>();                                   // strips: the first wait (in the prologue) sees every CTA of the cluster running
 
+  constexpr int HR = C::HALO ? 1 : 0;                    // shared arrays keep local row r at row r + HR
   Th th;
-  th.y = tl / C::TPR; th.j0 = (tl % C::TPR) * V;
-  th.row = 4u * (uint32_t)(th.y * C::Lh + th.j0);
-  th.rowp = 4u * (uint32_t)(((th.y + 1 == L) ? 0 : th.y + 1) * C::Lh + th.j0);
-  th.rowm = 4u * (uint32_t)(((th.y == 0) ? L - 1 : th.y - 1) * C::Lh + th.j0);
-  th.edge0 = 4u * (uint32_t)(th.y * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1));
-  th.edge1 = 4u * (uint32_t)(th.y * C::Lh + ((th.j0 + V == C::Lh) ? 0 : th.j0 + V));
+  const int ly = tl / C::TPR;
+  th.j0 = (tl % C::TPR) * V;
+  th.gy = sm.y0 + ly;
+  th.grow = th.gy * C::Lh + th.j0;
+  th.row = 4u * (uint32_t)((ly + HR) * C::Lh + th.j0);
+  if (C::HALO) {
+    th.rowp = th.row + 4u * C::Lh;
+    th.rowm = th.row - 4u * C::Lh;
+    th.edge = (ly == 0) ? -1 : (ly == YS - 1 ? 1 : 0);
+    const int hy = (th.gy + L + th.edge) % L;
+    th.grow_halo = hy * C::Lh + th.j0;
+    th.halo = th.edge < 0 ? th.rowm : th.rowp;
+    // the new colour-0 spins of an edge row are the neighbour strip's halo row on its far side
+    const uint32_t nb = (uint32_t)((rank + C::NCL + th.edge) % C::NCL);
+    const uint32_t nb_row = 4u * (uint32_t)((th.edge < 0 ? YS + 1 : 0) * C::Lh + th.j0);
+    th.push = th.edge != 0 ? mapa_u32(sm.x0 + nb_row, nb) : 0u;
+    th.push_bar = th.edge != 0 ? mapa_u32(sm.hfull, nb) : 0u;
+  } else {
+    th.rowp = 4u * (uint32_t)(((ly + 1 == L) ? 0 : ly + 1) * C::Lh + th.j0);
+    th.rowm = 4u * (uint32_t)(((ly == 0) ? L - 1 : ly - 1) * C::Lh + th.j0);
+    th.edge = 0; th.grow_halo = 0; th.halo = 0; th.push = 0; th.push_bar = 0;
+  }
+  th.edge0 = 4u * (uint32_t)((ly + HR) * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1));
+  th.edge1 = 4u * (uint32_t)((ly + HR) * C::Lh + ((th.j0 + V == C::Lh) ? 0 : th.j0 + V));
 
   const Geom& g = a.g;
-  const int slot = blockIdx.x * G + gs;                 // G consecutive slots of one sample
+  const int slot = group * G + gs;                      // G consecutive slots of one sample
   const int d = slot / (g.O * g.T);
   const int grp = slot / g.T;
   const int t = a.temp_of_slot[slot];
@@ -495,22 +655,24 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
   st.issued = -1; st.waited = -1;
   st.total = n_sweeps * L + 2;                          // planes L-1, 0, 1, ..., L-1, 0, 1, ... (index q -> plane (q-1) mod L)
   EAcc ea = {0.0, 0.0, 0.0, 0.0};
+  uint32_t hph = 0;                                     // phase parities of the two halo mbarriers
   const bool want_e = a.e_slot != nullptr;
   for (int s = 0; s < n_sweeps; ++s) {
     const bool fin = want_e && s + 1 == n_sweeps;       // the final sweep also reduces E and m
     if (s < a.n_or) {
       hp.c1 = 0; hp.c3 = 0;
-      if (fin) march_sweep<L, V, G, false, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
-      else march_sweep<L, V, G, false, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
+      if (fin) march_sweep<L, YS, V, G, false, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
+      else march_sweep<L, YS, V, G, false, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
     } else {
       const unsigned long long khb = a.k_hb + (unsigned long long)(s - a.n_or);
       hp.c1 = (uint32_t)(khb & 0xFFFFFFFFull); hp.c3 = counter_hi(khb, DOMAIN_HB);
-      if (fin) march_sweep<L, V, G, true, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
-      else march_sweep<L, V, G, true, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh);
+      if (fin) march_sweep<L, YS, V, G, true, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
+      else march_sweep<L, YS, V, G, true, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
     }
   }
+  step_wait<C>();                                        // strips: nobody pushes into this CTA any more
   if (want_e) {
-    // fixed-order reduction per system: lanes by shuffle, warps by one thread (deterministic)
+    // fixed-order reduction per system: lanes by shuffle, warps by one thread, strips by rank 0 (deterministic)
     constexpr int WPS = C::WPS, RW = C::RW;
     double v[4] = {ea.e, ea.mx, ea.my, ea.mz};
     double* red = reinterpret_cast<double*>(smem_raw + C::red_off);
@@ -524,9 +686,20 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
       for (int i = 0; i < 4; ++i) red[(gs * WPS + tl / RW) * 4 + i] = v[i];
     }
     __syncthreads();
-    if (tl < 4) {
-      double x = 0.0;
+    double x = 0.0;
+    if (tl < 4)
       for (int w = 0; w < WPS; ++w) x += red[(gs * WPS + w) * 4 + tl];
+    if (C::HALO) {
+      if (tl < 4) st_cluster_f64(mapa_u32(base + C::red2_off + 8u * (uint32_t)((gs * C::NCL + rank) * 4 + tl), 0u), x);
+      cluster_arrive();
+      cluster_wait();
+      if (rank == 0 && tl < 4) {
+        const double* red2 = reinterpret_cast<const double*>(smem_raw + C::red2_off);
+        x = 0.0;
+        for (int r = 0; r < C::NCL; ++r) x += red2[(gs * C::NCL + r) * 4 + tl];
+      }
+    }
+    if (rank == 0 && tl < 4) {
       if (tl == 0) a.e_slot[slot] = -x;
       else a.m_slot[slot * 3 + (tl - 1)] = x / (double)g.N;
     }
@@ -536,17 +709,29 @@ __global__ void __launch_bounds__(Cfg<L, V, G>::NT, 1) zmarch_kernel(ZmarchArgs 
 }  // namespace zm
 
 // ------------------------------------------------------------------------------------------------ host side
-template <int L, int V, int G>
+template <int L, int YS, int V, int G>
 inline cudaError_t zmarch_launch_t(const ZmarchArgs& a, cudaStream_t stream) {
-  using C = zm::Cfg<L, V, G>;
+  using C = zm::Cfg<L, YS, V, G>;
   static bool configured = false;
   if (!configured) {
-    const cudaError_t e = cudaFuncSetAttribute(zm::zmarch_kernel<L, V, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+    const cudaError_t e = cudaFuncSetAttribute(zm::zmarch_kernel<L, YS, V, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
     if (e != cudaSuccess) return e;
     configured = true;
   }
-  zm::zmarch_kernel<L, V, G><<<a.g.R / G, C::NT, C::smem_bytes, stream>>>(a);
-  return cudaGetLastError();
+  if (C::NCL == 1) {
+    zm::zmarch_kernel<L, YS, V, G><<<a.g.R / G, C::NT, C::smem_bytes, stream>>>(a);
+    return cudaGetLastError();
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(a.g.R / G * C::NCL));
+  cfg.blockDim = dim3(C::NT);
+  cfg.dynamicSmemBytes = C::smem_bytes;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = C::NCL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, zm::zmarch_kernel<L, YS, V, G>, a);
 }
 
 // largest group size the geometry allows: the G slots of a CTA must belong to one sample
@@ -556,28 +741,34 @@ inline int zmarch_pick_g(const Geom& g, int gmax) {
   return G;
 }
 
-inline bool zmarch_supported(const Geom& g) { return g.L == 8 || g.L == 16 || g.L == 32; }
+inline bool zmarch_supported(const Geom& g) { return g.L == 8 || g.L == 16 || g.L == 32 || g.L == 64; }
 
-#define HSG_ZM_CASE(L_, V_, G_) if (a.g.L == L_ && G == G_) return zmarch_launch_t<L_, V_, G_>(a, stream);
+#define HSG_ZM_CASE(L_, YS_, V_, G_) if (a.g.L == L_ && G == G_) return zmarch_launch_t<L_, YS_, V_, G_>(a, stream);
 inline cudaError_t zmarch_launch(const ZmarchArgs& a, cudaStream_t stream, int* n_launch) {
   *n_launch = 1;
   if (a.g.L == 32) {
     const int G = zmarch_pick_g(a.g, HSG_ZM_L32_G);
-    HSG_ZM_CASE(32, HSG_ZM_L32_V, HSG_ZM_L32_G)
+    HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, HSG_ZM_L32_G)
 #if HSG_ZM_L32_G > 2
-    HSG_ZM_CASE(32, HSG_ZM_L32_V, 2)
+    HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, 2)
 #endif
 #if HSG_ZM_L32_G > 1
-    HSG_ZM_CASE(32, HSG_ZM_L32_V, 1)
+    HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, 1)
 #endif
   }
-#ifndef HSG_ZM_ONLY_L32     // (variant builds for experiments instantiate L = 32 only)
+#ifndef HSG_ZM_NO_L64
+  else if (a.g.L == 64) {      // four strips of 16 rows = a cluster of four CTAs per group of two systems
+    const int G = zmarch_pick_g(a.g, 2);
+    HSG_ZM_CASE(64, 16, 4, 2) HSG_ZM_CASE(64, 16, 4, 1)
+  }
+#endif
+#ifndef HSG_ZM_ONLY_L32     // (variant builds for experiments instantiate L = 32 and 64 only)
   else if (a.g.L == 16) {
     const int G = zmarch_pick_g(a.g, 8);
-    HSG_ZM_CASE(16, HSG_ZM_L16_V, 8) HSG_ZM_CASE(16, HSG_ZM_L16_V, 4) HSG_ZM_CASE(16, HSG_ZM_L16_V, 2) HSG_ZM_CASE(16, HSG_ZM_L16_V, 1)
+    HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 8) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 4) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 2) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 1)
   } else if (a.g.L == 8) {
     const int G = zmarch_pick_g(a.g, 8);
-    HSG_ZM_CASE(8, 2, 8) HSG_ZM_CASE(8, 2, 4) HSG_ZM_CASE(8, 2, 2) HSG_ZM_CASE(8, 2, 1)
+    HSG_ZM_CASE(8, 8, 2, 8) HSG_ZM_CASE(8, 8, 2, 4) HSG_ZM_CASE(8, 8, 2, 2) HSG_ZM_CASE(8, 8, 2, 1)
   }
 #endif
   *n_launch = 0;

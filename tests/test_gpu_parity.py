@@ -44,7 +44,7 @@ def test_init_spins_bit_exact(L, D, O, T):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("L,D,O,T", [(4, 1, 1, 1), (6, 2, 1, 2), (8, 1, 2, 16), (10, 1, 2, 3), (12, 2, 2, 2), (16, 3, 2, 4), (32, 1, 2, 4)])
+@pytest.mark.parametrize("L,D,O,T", [(4, 1, 1, 1), (6, 2, 1, 2), (8, 1, 2, 16), (10, 1, 2, 3), (12, 2, 2, 2), (16, 3, 2, 4), (32, 1, 2, 4), (64, 1, 2, 2), (64, 2, 1, 1)])
 def test_or_sweeps_bit_exact(kernel, L, D, O, T):
     """Over-relaxation (Eq. 3) is deterministic arithmetic: the trajectory must agree to the last bit."""
     eng, orc = _pair(L, D, O, T, seed=5, kernel=kernel)
@@ -56,7 +56,7 @@ def test_or_sweeps_bit_exact(kernel, L, D, O, T):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("L,D,O,T", [(4, 1, 1, 2), (6, 1, 2, 2), (8, 1, 2, 16), (12, 2, 1, 3), (16, 2, 2, 4), (32, 1, 2, 4)])
+@pytest.mark.parametrize("L,D,O,T", [(4, 1, 1, 2), (6, 1, 2, 2), (8, 1, 2, 16), (12, 2, 1, 3), (16, 2, 2, 4), (32, 1, 2, 4), (64, 1, 2, 2)])
 def test_hb_sweeps_bit_exact(kernel, L, D, O, T):
     """Heat bath (Eq. 2) with the fixed series of DESIGN.md §3.4 and the same Philox draws."""
     eng, orc = _pair(L, D, O, T, seed=6, kernel=kernel, sample_offset=2)
@@ -69,7 +69,7 @@ def test_hb_sweeps_bit_exact(kernel, L, D, O, T):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("cfg,D", [("c1", 1), ("c2", 2), ("c3", 2), ("c4", 1)])
+@pytest.mark.parametrize("cfg,D", [("c1", 1), ("c2", 2), ("c3", 2), ("c4", 1), ("c5", 1)])
 def test_ten_sweeps_of_the_baseline_configs(kernel, cfg, D):
     """BASELINE.json: per-component spin difference <= 1e-4 after 10 sweeps (cold start, OR then HB)."""
     c, temps, J, H = hsg_inputs.make_config(cfg, n_samples=D)
@@ -243,7 +243,7 @@ def test_branch_free_division_and_sqrt_are_ieee_correct():
     assert hsg.hsg_selftest_arith(200_000_000, seed=12345) == (0, 0)
 
 
-@pytest.mark.parametrize("L,D,O,T", [(8, 1, 2, 16), (16, 2, 2, 4), (32, 1, 2, 4)])
+@pytest.mark.parametrize("L,D,O,T", [(8, 1, 2, 16), (16, 2, 2, 4), (32, 1, 2, 4), (64, 1, 2, 2), (64, 1, 1, 1)])
 @pytest.mark.parametrize("n_or,n_hb", [(1, 0), (3, 0), (0, 1), (2, 2)])
 def test_energy_fused_into_the_last_sweep_matches_oracle_and_the_separate_reduction(L, D, O, T, n_or, n_hb):
     """the z-marching kernel reduces E and m in the final sweep of a call (OR or HB)."""
