@@ -337,11 +337,15 @@ int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, doub
   const int P = g.O * (g.O - 1) / 2;
   if ((q0_dev || qk_dev) && P > 0) {
     const long long n_sys = (long long)g.D * P * g.T;
-    const int V = vec_width(g), ZB = reduce_zb(g, V), n_chunks = (g.L + ZB - 1) / ZB;
+    // a block takes whole systems (chunks of 16 planes at L = 64) with enough (y,z) rows per thread to amortise the
+    // per-pass phase fold: about 8 rows per thread and x-parity, at least one warp, at most kThreads
+    const int V = vec_width(g), ZB = g.L > 32 ? 16 : g.L, n_chunks = (g.L + ZB - 1) / ZB;
     const unsigned nb = (unsigned)(n_sys * n_chunks);
-    if (V == 4) overlap_kernel<4><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
-    else if (V == 2) overlap_kernel<2><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
-    else overlap_kernel<1><<<nb, kThreads, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+    int nt = 32;
+    while (nt < kThreads && ((long long)ZB * g.L * (g.Lh / V) >= 8LL * nt || nt < 2 * (g.Lh / V))) nt *= 2;
+    if (V == 4) overlap_kernel<4><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+    else if (V == 2) overlap_kernel<2><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+    else overlap_kernel<1><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
     HSG_LAUNCHED(ctx);
     finalize_overlap_kernel<<<blocks_for(n_sys * 9), kThreads, 0, ctx->stream>>>(g, (int)n_sys, n_chunks, ctx->q_partial, q0_dev, qk_dev);
     HSG_LAUNCHED(ctx);

@@ -346,10 +346,13 @@ __global__ void pt_swap_kernel(Geom g, PhiloxKey key, unsigned long long k_pt, c
 }
 
 // ------------------------------------------------------------------ overlap tensor, Eqs. (5), (6)
-// One block per (d, pair, t, chunk of ZB planes): partial[(d,p,t)][chunk][27] = 9 sums for k=0, 9 re, 9 im
-// for k_min.  Each thread takes items of V compact sites (vector loads of both replicas).
+// One block per (d, pair, t, chunk of ZB planes): partial[(d,p,t)][chunk][27] = 9 sums for k=0, 9 re, 9 im for k_min.
+// k_min lies along x, so  sum_i a_i b_i e^{ikx_i} = sum_x e^{ikx} [ sum_{y,z} a b ]:  a thread keeps a fixed group of
+// V compact sites j0..j0+V-1 and ONE x-parity, accumulates the nine products of every (y,z) row it visits (sites of
+// x = 2(j0+e) + parity) and applies the phase once at the end.  9 fp64 FMAs per site instead of 27.
+// blockDim.x may be smaller than kThreads (small lattices); threads beyond 2*RT*qpr idle.
 template <int V>
-__global__ void __launch_bounds__(kThreads) overlap_kernel(Geom g, int ZB, const float* __restrict__ spins, const int32_t* __restrict__ slot_of_temp,
+__global__ void __launch_bounds__(kThreads, 2) overlap_kernel(Geom g, int ZB, const float* __restrict__ spins, const int32_t* __restrict__ slot_of_temp,
                                                            const double* __restrict__ cs_table /*[L][2]*/, double* __restrict__ partial) {
   const int L = g.L, Lh = g.Lh, qpr = Lh / V;
   const int P = g.O * (g.O - 1) / 2;
@@ -365,40 +368,67 @@ __global__ void __launch_bounds__(kThreads) overlap_kernel(Geom g, int ZB, const
   const float* A = spins + (long long)sa * 3 * g.N;
   const float* B = spins + (long long)sb * 3 * g.N;
   const int z0 = chunk * ZB, nz = min(ZB, L - z0);
+  const int RT = (int)blockDim.x / (2 * qpr);     // row lanes per x-parity
+  const int q = (int)threadIdx.x % qpr, par = ((int)threadIdx.x / qpr) & 1, r = (int)threadIdx.x / (2 * qpr), j0 = q * V;
   double acc[27];
 #pragma unroll
   for (int k = 0; k < 27; ++k) acc[k] = 0.0;
-  const int ipp = 2 * L * qpr;
-  for (int it = threadIdx.x; it < nz * ipp; it += kThreads) {
-    const int q = it % qpr; int rem = it / qpr;
-    const int y = rem % L; rem /= L;
-    const int c = rem & 1; const int z = z0 + (rem >> 1);
-    const int j0 = q * V;
-    const int off = (y + z + c) & 1;
-    Vec<V> av[3], bv[3];
+  if (r < RT) {
+    {
+      double s9[V][9];
 #pragma unroll
-    for (int mu = 0; mu < 3; ++mu) {
-      av[mu] = ldv<V>(A + spin_index(g, z, c, mu, y, j0));
-      bv[mu] = ldv<V>(B + spin_index(g, z, c, mu, y, j0));
-    }
+      for (int e = 0; e < V; ++e)
 #pragma unroll
-    for (int e = 0; e < V; ++e) {
-      const int x = 2 * (j0 + e) + off;
-      const double co = cs_table[2 * x], si = cs_table[2 * x + 1];
-      double ad[3], bd[3], bc[3], bs[3];
+        for (int k = 0; k < 9; ++k) s9[e][k] = 0.0;
+      for (int m = r; m < nz * L; m += RT) {
+        const int y = m % L, z = z0 + m / L;
+        const int c = (par + y + z) & 1;    // the colour whose sites of row (y,z) sit at x = 2j + par
+        Vec<V> av[3], bv[3];
 #pragma unroll
-      for (int mu = 0; mu < 3; ++mu) { ad[mu] = (double)av[mu].v[e]; bd[mu] = (double)bv[mu].v[e]; bc[mu] = bd[mu] * co; bs[mu] = bd[mu] * si; }
-#pragma unroll
-      for (int mu = 0; mu < 3; ++mu)
-#pragma unroll
-        for (int nu = 0; nu < 3; ++nu) {
-          acc[mu * 3 + nu] = fma(ad[mu], bd[nu], acc[mu * 3 + nu]);
-          acc[9 + mu * 3 + nu] = fma(ad[mu], bc[nu], acc[9 + mu * 3 + nu]);
-          acc[18 + mu * 3 + nu] = fma(ad[mu], bs[nu], acc[18 + mu * 3 + nu]);
+        for (int mu = 0; mu < 3; ++mu) {
+          av[mu] = ldv<V>(A + spin_index(g, z, c, mu, y, j0));
+          bv[mu] = ldv<V>(B + spin_index(g, z, c, mu, y, j0));
         }
+#pragma unroll
+        for (int e = 0; e < V; ++e) {
+          double ad[3], bd[3];
+#pragma unroll
+          for (int mu = 0; mu < 3; ++mu) { ad[mu] = (double)av[mu].v[e]; bd[mu] = (double)bv[mu].v[e]; }
+#pragma unroll
+          for (int mu = 0; mu < 3; ++mu)
+#pragma unroll
+            for (int nu = 0; nu < 3; ++nu) s9[e][mu * 3 + nu] = fma(ad[mu], bd[nu], s9[e][mu * 3 + nu]);
+        }
+      }
+#pragma unroll
+      for (int e = 0; e < V; ++e) {
+        const int x = 2 * (j0 + e) + par;
+        const double co = cs_table[2 * x], si = cs_table[2 * x + 1];
+#pragma unroll
+        for (int k = 0; k < 9; ++k) {
+          acc[k] += s9[e][k];
+          acc[9 + k] = fma(s9[e][k], co, acc[9 + k]);
+          acc[18 + k] = fma(s9[e][k], si, acc[18 + k]);
+        }
+      }
     }
   }
-  block_reduce_store<27>(acc, partial + (long long)blockIdx.x * 27);
+  // fixed-order block reduction over the warps that exist in this launch
+  __shared__ double sm[kThreads / 32][27];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = ((int)blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int k = 0; k < 27; ++k) {
+    double x = acc[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    if (lane == 0) sm[warp][k] = x;
+  }
+  __syncthreads();
+  if (threadIdx.x < 27) {
+    double x = 0.0;
+    for (int w = 0; w < n_warps; ++w) x += sm[w][threadIdx.x];
+    partial[(long long)blockIdx.x * 27 + threadIdx.x] = x;
+  }
 }
 
 __global__ void finalize_overlap_kernel(Geom g, int n_sys /*D*P*T*/, int n_chunks, const double* __restrict__ partial, double* __restrict__ q0, double* __restrict__ qk) {

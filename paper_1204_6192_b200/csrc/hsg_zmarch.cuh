@@ -203,6 +203,7 @@ template <int L, int YS, int V, int G> struct Cfg {
   static constexpr int HPS = 3 * CSS;
   static constexpr int CSJ = (YS + (HALO ? 1 : 0)) * Lh;   // shared J/H array: halo row below (for the -y couplings), YS rows
   static constexpr int JA = 11 * CSJ;             // ring A slot: 11 arrays; ring B slot: colour-0 Jz
+  static constexpr int NJA = kNJA, NJB = kNJB;    // J/H ring depths (ring_advance)
   static constexpr int RW = TPS < 32 ? TPS : 32;  // shuffle width of the per-system reduction
   static constexpr int WPS = TPS / RW;            // partial sums per system after the shuffle stage
   // byte offsets inside dynamic shared memory
@@ -357,16 +358,16 @@ struct Stream {        // J/H plane stream: index q -> plane (q-1) mod L
 // Slot reuse is safe because the barrier that ended the previous step separates the last reads of index
 // nd-2 (ring A) and nd-3 (ring B) from the copies issued here.  Whole-plane CTAs move a plane with two bulk copies;
 // strip CTAs move the YS rows of each of the twelve arrays plus the halo row of the two Jy arrays (14 copies, one per lane).
-template <class C, int L>
-__device__ __forceinline__ void ring_advance(const Smem& sm, const float* __restrict__ jh_d, Stream& st, int nd, uint64_t pol) {
+template <class C, int L, class SmemT>
+__device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __restrict__ jh_d, Stream& st, int nd, uint64_t pol) {
   constexpr uint32_t JAB = 4u * C::JA, JBB = 4u * C::CSJ;
   if (threadIdx.x < 32) {
     const int upto = min(nd + kDJ, st.total - 1);
     while (st.issued < upto) {
       ++st.issued;
       const int plane = (st.issued + L - 1) % L;
-      const uint32_t bar = sm.full + 8u * ((uint32_t)st.issued % kNJB);
-      const uint32_t dA = sm.ja + ((uint32_t)st.issued % kNJA) * JAB, dB = sm.jb + ((uint32_t)st.issued % kNJB) * JBB;
+      const uint32_t bar = sm.full + 8u * ((uint32_t)st.issued % C::NJB);
+      const uint32_t dA = sm.ja + ((uint32_t)st.issued % C::NJA) * JAB, dB = sm.jb + ((uint32_t)st.issued % C::NJB) * JBB;
       const float* src = jh_d + (size_t)plane * 12 * C::CSG;
       if (!C::HALO) {
         if (threadIdx.x == 0) {
@@ -396,8 +397,8 @@ __device__ __forceinline__ void ring_advance(const Smem& sm, const float* __rest
   }
   while (st.waited < nd) {
     ++st.waited;
-    const uint32_t bar = sm.full + 8u * ((uint32_t)st.waited % kNJB);
-    const uint32_t parity = ((uint32_t)st.waited / kNJB) & 1u;
+    const uint32_t bar = sm.full + 8u * ((uint32_t)st.waited % C::NJB);
+    const uint32_t parity = ((uint32_t)st.waited / C::NJB) & 1u;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
