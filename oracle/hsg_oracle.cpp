@@ -323,10 +323,14 @@ struct Sim {
         Real h[3], cur[3] = { s[i], s[N + i], s[2 * N + i] }, out[3];
         local_field(s, Jd, Hd, i, h);
         if (heat_bath) {
+          // one Philox call serves the two same-colour sites x and x+2 whose compact index
+          // j = x>>1 is (even, odd): counter word 0 = the site with even j; that site takes output words 0, 1,
+          // its partner words 2, 3.
+          const int odd = (x >> 1) & 1;
           uint32_t ctr[4], w[4];
-          make_counter((uint32_t)i, k_hb, sid, DOMAIN_HB, ctr);
+          make_counter((uint32_t)(i - 2 * odd), k_hb, sid, DOMAIN_HB, ctr);
           philox4x32_10(ctr, k, w);
-          hb_draw<Real>(h, b, u01<Real>(w[0]), u01<Real>(w[1]), out);
+          hb_draw<Real>(h, b, u01<Real>(w[2 * odd]), u01<Real>(w[2 * odd + 1]), out);
         } else {
           or_reflect<Real>(cur, h, out);
         }

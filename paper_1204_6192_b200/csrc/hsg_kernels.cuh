@@ -193,13 +193,23 @@ __global__ void __launch_bounds__(kThreads) sweep_generic_kernel(SweepArgs a, in
     const int grp = slot / g.T;
     const uint32_t sysid = (uint32_t)((g.sample_offset * g.O * g.T) + (unsigned long long)grp * g.T + t);
     const uint32_t c1 = (uint32_t)(a.k_hb & 0xFFFFFFFFull), c3 = counter_hi(a.k_hb, DOMAIN_HB);
+    // one Philox call per pair of same-colour sites with compact index (even, odd): counter word 0 = the even one,
+    // which takes output words 0, 1; its partner takes words 2, 3.  V = 1: every thread makes the call.
+    uint32_t wa[V], wb[V];
+    if (V == 1) {
+      const int odd = j0 & 1;
+      uint32_t w0, w1, w2, w3;
+      philox4x32_10((uint32_t)(2 * (j0 - odd) + off + L * (y + L * z)), c1, sysid, c3, a.key.k0, a.key.k1, w0, w1, w2, w3);
+      wa[0] = odd ? w2 : w0; wb[0] = odd ? w3 : w1;
+    } else {
+#pragma unroll
+      for (int e = 0; e + 1 < V; e += 2)
+        philox4x32_10((uint32_t)(2 * (j0 + e) + off + L * (y + L * z)), c1, sysid, c3, a.key.k0, a.key.k1, wa[e], wb[e], wa[e + 1 < V ? e + 1 : e], wb[e + 1 < V ? e + 1 : e]);
+    }
 #pragma unroll
     for (int e = 0; e < V; ++e) {
-      const uint32_t site = (uint32_t)(2 * (j0 + e) + off + L * (y + L * z));
-      uint32_t w0, w1, w2, w3;
-      philox4x32_10(site, c1, sysid, c3, a.key.k0, a.key.k1, w0, w1, w2, w3);
       const Vec3 hv = { h[0][e], h[1][e], h[2][e] };
-      const Vec3 s = hb_draw(hv, beta, u01(w0), u01(w1));
+      const Vec3 s = hb_draw(hv, beta, u01(wa[e]), u01(wb[e]));
       out[0].v[e] = s.x; out[1].v[e] = s.y; out[2].v[e] = s.z;
     }
   } else {

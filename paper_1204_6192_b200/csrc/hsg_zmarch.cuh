@@ -60,6 +60,9 @@ namespace zm {
 #ifndef HSG_ZM_L32_G
 #define HSG_ZM_L32_G 2
 #endif
+#ifndef HSG_ZM_L32_VHB
+#define HSG_ZM_L32_VHB 2         // L = 32: sites per thread in the heat-bath phase (0: same launch as the over-relaxation phase)
+#endif
 #ifndef HSG_ZM_L16_V
 #define HSG_ZM_L16_V 4
 #endif
@@ -214,7 +217,7 @@ template <int L, int YS, int V, int G> struct Cfg {
   static constexpr uint32_t sys_off = jb_off + 4u * kNJB * CSJ;
   static constexpr uint32_t sys_bytes = 4u * (kNC1 + kNC0 + 2) * HPS;    // per system: C1 ring, C0 ring, X0[2]
   static constexpr size_t smem_bytes = sys_off + (size_t)G * sys_bytes;
-  static_assert(L % YS == 0 && Lh % V == 0, "strip height divides L, vector width divides the row length");
+  static_assert(L % YS == 0 && Lh % V == 0 && V % 2 == 0, "strip height divides L, even vector width divides the row length");
   static_assert((YS * Lh * 4) % 16 == 0 && (Lh * 4) % 16 == 0, "bulk copies move multiples of 16 bytes");
   static_assert(!HALO || V == 4, "halo copies use 16-byte cp.async.cg");
   static_assert(!HALO || YS >= 2, "a thread is on at most one strip edge");
@@ -312,14 +315,20 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
       }
     }
   }
+  // heat bath: one Philox call per pair of sites (e, e+1), e even: counter word 0 = the site with even compact index
+  // (j0 is a multiple of V), which takes output words 0, 1; its partner takes words 2, 3
+  uint32_t wa[V], wb[V];
+  if (HB) {
+#pragma unroll
+    for (int e = 0; e < V; e += 2)
+      philox4x32_10(site0 + 2u * (uint32_t)e, hp.c1, hp.sysid, hp.c3, hp.key.k0, hp.key.k1, wa[e], wb[e], wa[e + 1], wb[e + 1]);
+  }
 #pragma unroll
   for (int e = 0; e < V; ++e) {
     const Vec3 hv = {h[0][e], h[1][e], h[2][e]};
     Vec3 s;
     if (HB) {
-      uint32_t w0, w1, w2, w3;
-      philox4x32_10(site0 + 2u * (uint32_t)e, hp.c1, hp.sysid, hp.c3, hp.key.k0, hp.key.k1, w0, w1, w2, w3);
-      s = hb_draw(hv, hp.beta, u01(w0), u01(w1));
+      s = hb_draw(hv, hp.beta, u01(wa[e]), u01(wb[e]));
     } else {
       const Vec3 sv = {own[0][e], own[1][e], own[2][e]};
       s = or_reflect(sv, hv);
@@ -749,6 +758,22 @@ inline cudaError_t zmarch_launch(const ZmarchArgs& a, cudaStream_t stream, int* 
   *n_launch = 1;
   if (a.g.L == 32) {
     const int G = zmarch_pick_g(a.g, HSG_ZM_L32_G);
+#if HSG_ZM_L32_VHB > 0
+    // The heat-bath sweeps are bound by instruction issue, the over-relaxation sweeps by memory: the heat-bath phase
+    // runs as a launch of its own with half the sites (and registers) per thread and twice the warps per SM.
+    if (G == HSG_ZM_L32_G && a.n_hb > 0) {
+      if (a.n_or > 0) {
+        ZmarchArgs o = a;
+        o.n_hb = 0; o.e_slot = nullptr;
+        const cudaError_t e = zmarch_launch_t<32, 32, HSG_ZM_L32_V, HSG_ZM_L32_G>(o, stream);
+        if (e != cudaSuccess) return e;
+        *n_launch = 2;
+      }
+      ZmarchArgs h = a;
+      h.n_or = 0;
+      return zmarch_launch_t<32, 32, HSG_ZM_L32_VHB, HSG_ZM_L32_G>(h, stream);
+    }
+#endif
     HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, HSG_ZM_L32_G)
 #if HSG_ZM_L32_G > 2
     HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, 2)

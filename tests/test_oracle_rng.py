@@ -77,3 +77,40 @@ def test_init_spins_follow_the_documented_counter_packing():
     assert np.abs(Sb.mean(axis=1)).max() < 4 * np.sqrt(1 / 3 / n)
     assert np.abs((Sb**2).mean(axis=1) - 1 / 3).max() < 4 * np.sqrt(4 / 45 / n)
     np.testing.assert_allclose((Sb**2).sum(axis=0), 1.0, atol=3e-7)
+
+
+def test_heat_bath_sweep_follows_the_documented_counter_packing():
+    """HB: c1/c3 = sweep counter k_hb with DOMAIN_HB, c2 = ((off+d)*O+o)*T+t, and ONE Philox call per
+    pair of same-colour sites x, x+2 with compact index j = x>>1 (even, odd): c0 = index of the even-j site, which takes
+    words 0,1; its partner takes words 2,3.  Checked on a lattice without couplings, where the local field is H_i, so
+    every new spin is hb_draw(H_i, beta_t, u1, u2) of exactly those two words — for two successive sweeps."""
+    for Lx in (4, 6):                                   # Lh even and odd (unpaired last site of a row)
+        D, O, T, seed, off = 2, 2, 2, 0xFEDCBA98_76543210, 3
+        temps = np.array([0.5, 0.9], dtype=np.float32)
+        N = Lx**3
+        rng = np.random.default_rng(5)
+        J = np.zeros((D, 3, Lx, Lx, Lx), dtype=np.float32)
+        H = rng.standard_normal((D, 3, Lx, Lx, Lx)).astype(np.float32)
+        sim = oracle.Oracle(Lx, D, O, temps, seed, precision=64, sample_offset=off)
+        sim.set_disorder(J, H)
+        sim.init_spins()
+        site = np.arange(N)
+        x = site % Lx
+        odd = (x >> 1) & 1
+        c0 = site - 2 * odd
+        for k_hb in range(2):
+            sim.sweep(0, 1)
+            S = sim.get_spins().reshape(D, O, T, 3, N)
+            for d in range(D):
+                for o in range(O):
+                    for t in range(T):
+                        sysid = ((off + d) * O + o) * T + t
+                        w = pnp.draw(pnp.DOMAIN_HB, c0, k_hb, sysid, seed)
+                        u1 = np.where(odd == 1, pnp.u01(w[2]), pnp.u01(w[0]))
+                        u2 = np.where(odd == 1, pnp.u01(w[3]), pnp.u01(w[1]))
+                        beta = float(np.float32(1.0 / np.float64(temps[t])))
+                        Hd = H[d].reshape(3, N).astype(np.float64)
+                        for i in range(0, N, 7):        # a sample of the sites, every residue of x
+                            ref = oracle.hb_draw(Hd[:, i], beta, u1[i], u2[i], precision=64)
+                            np.testing.assert_allclose(S[d, o, t, :, i], ref, atol=1e-14)
+        assert sim.get_state()[1][0] == 2
