@@ -63,6 +63,9 @@ namespace zm {
 #ifndef HSG_ZM_L32_VHB
 #define HSG_ZM_L32_VHB 2         // L = 32: sites per thread in the heat-bath phase (0: same launch as the over-relaxation phase)
 #endif
+#ifndef HSG_ZM_L16_VHB
+#define HSG_ZM_L16_VHB 2
+#endif
 #ifndef HSG_ZM_L16_V
 #define HSG_ZM_L16_V 4
 #endif
@@ -791,6 +794,20 @@ inline cudaError_t zmarch_launch(const ZmarchArgs& a, cudaStream_t stream, int* 
 #ifndef HSG_ZM_ONLY_L32     // (variant builds for experiments instantiate L = 32 and 64 only)
   else if (a.g.L == 16) {
     const int G = zmarch_pick_g(a.g, 8);
+#if HSG_ZM_L16_VHB > 0
+    if (G == 8 && a.n_hb > 0) {     // heat-bath phase as its own launch with twice the warps, as at L = 32
+      if (a.n_or > 0) {
+        ZmarchArgs o = a;
+        o.n_hb = 0; o.e_slot = nullptr;
+        const cudaError_t e = zmarch_launch_t<16, 16, HSG_ZM_L16_V, 8>(o, stream);
+        if (e != cudaSuccess) return e;
+        *n_launch = 2;
+      }
+      ZmarchArgs h = a;
+      h.n_or = 0;
+      return zmarch_launch_t<16, 16, HSG_ZM_L16_VHB, 8>(h, stream);
+    }
+#endif
     HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 8) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 4) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 2) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 1)
   } else if (a.g.L == 8) {
     const int G = zmarch_pick_g(a.g, 8);
