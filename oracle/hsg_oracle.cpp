@@ -360,21 +360,22 @@ struct Sim {
     }
   }
 
-  // PAPER.md:26 Eq. (1), each nearest-neighbour bond once (reading 1); products and sum in double.
+  // PAPER.md:26 Eq. (1), each nearest-neighbour bond once (reading 1), in the bipartite form: every bond joins an
+  // even and an odd site, so  E = - sum_{i odd} s_i . h_i  -  sum_{i even} s_i . H_i  with h_i = H_i + sum_j J_ij s_j
+  // the local field of the moves.  Site terms in the spins' precision Real with the fixed FMA order of
+  // the moves, the sum over sites in double ("spins ... single precision and aggregate quantities ...
+  // double precision", reading 11).
   double energy_of(const Real* s, int d) const {
     const float* Jd = &J[(size_t)d * 3 * N];
     const float* Hd = &H[(size_t)d * 3 * N];
     double E = 0.0;
-    for (long i = 0; i < N; ++i) {
-      const double sx = (double)s[i], sy = (double)s[N + i], sz = (double)s[2 * N + i];
-      double acc = 0.0;
-      for (int dir = 0; dir < 3; ++dir) {
-        const long ip = nbr(i, dir, +1);
-        const double dot = sx * (double)s[ip] + sy * (double)s[N + ip] + sz * (double)s[2 * N + ip];
-        acc += (double)Jd[(size_t)dir * N + i] * dot;
-      }
-      acc += (double)Hd[i] * sx + (double)Hd[N + i] * sy + (double)Hd[2 * N + i] * sz;
-      E -= acc;
+    for (int z = 0; z < L; ++z) for (int y = 0; y < L; ++y) for (int x = 0; x < L; ++x) {
+      const long i = x + (long)L * (y + (long)L * z);
+      Real h[3];
+      if ((x + y + z) & 1) local_field(s, Jd, Hd, i, h);
+      else for (int c = 0; c < 3; ++c) h[c] = (Real)Hd[(size_t)c * N + i];
+      const Real e = fma_(s[2 * N + i], h[2], fma_(s[N + i], h[1], s[i] * h[0]));
+      E -= (double)e;
     }
     return E;
   }

@@ -118,6 +118,52 @@ struct SweepArgs {
   unsigned long long k_hb;      // heat-bath sweep counter of THIS sweep
 };
 
+// Local field of the V compact sites j0..j0+V-1 of colour c in row (y,z), straight from global memory:
+// h = H, then x+, x-, y+, y-, z+, z- in that order, one explicit FMA each.
+template <int V>
+__device__ __forceinline__ void local_field_global(const Geom& g, const float* __restrict__ S, const float* __restrict__ JH,
+                                                   int z, int c, int y, int j0, float (&h)[3][V]) {
+  const int L = g.L, Lh = g.Lh, cc = 1 - c;
+  const int off = (y + z + c) & 1;
+  const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
+  const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
+  const int jx = off ? ((j0 + V == Lh) ? 0 : j0 + V) : ((j0 == 0) ? Lh - 1 : j0 - 1);   // the one x-neighbour outside [j0, j0+V)
+  // couplings: forward bonds of this site, backward bonds stored at the neighbour
+  const Vec<V> Jxp = ldv<V>(JH + jh_index(g, z, c, 0, y, j0));
+  const Vec<V> Jyp = ldv<V>(JH + jh_index(g, z, c, 1, y, j0));
+  const Vec<V> Jzp = ldv<V>(JH + jh_index(g, z, c, 2, y, j0));
+  const Vec<V> Jxq = ldv<V>(JH + jh_index(g, z, cc, 0, y, j0));
+  const float Jxe = JH[jh_index(g, z, cc, 0, y, jx)];
+  const Vec<V> Jym = ldv<V>(JH + jh_index(g, z, cc, 1, ym, j0));
+  const Vec<V> Jzm = ldv<V>(JH + jh_index(g, zm, cc, 2, y, j0));
+  Vec<V> Jxm;
+#pragma unroll
+  for (int e = 0; e < V; ++e) Jxm.v[e] = off ? Jxq.v[e] : (e > 0 ? Jxq.v[e > 0 ? e - 1 : 0] : Jxe);
+#pragma unroll
+  for (int mu = 0; mu < 3; ++mu) {
+    const Vec<V> Hm = ldv<V>(JH + jh_index(g, z, c, 3 + mu, y, j0));
+    const Vec<V> sq = ldv<V>(S + spin_index(g, z, cc, mu, y, j0));
+    const float se = S[spin_index(g, z, cc, mu, y, jx)];
+    const Vec<V> syp = ldv<V>(S + spin_index(g, z, cc, mu, yp, j0));
+    const Vec<V> sym = ldv<V>(S + spin_index(g, z, cc, mu, ym, j0));
+    const Vec<V> szp = ldv<V>(S + spin_index(g, zp, cc, mu, y, j0));
+    const Vec<V> szm = ldv<V>(S + spin_index(g, zm, cc, mu, y, j0));
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+      const float sxp = off ? (e + 1 < V ? sq.v[e + 1 < V ? e + 1 : 0] : se) : sq.v[e];
+      const float sxm = off ? sq.v[e] : (e > 0 ? sq.v[e > 0 ? e - 1 : 0] : se);
+      float acc = Hm.v[e];
+      acc = __fmaf_rn(Jxp.v[e], sxp, acc);
+      acc = __fmaf_rn(Jxm.v[e], sxm, acc);
+      acc = __fmaf_rn(Jyp.v[e], syp.v[e], acc);
+      acc = __fmaf_rn(Jym.v[e], sym.v[e], acc);
+      acc = __fmaf_rn(Jzp.v[e], szp.v[e], acc);
+      acc = __fmaf_rn(Jzm.v[e], szm.v[e], acc);
+      h[mu][e] = acc;
+    }
+  }
+}
+
 // Each thread updates V consecutive compact sites of colour `colour` in one row (y,z) of one slot.
 // Neighbours are read straight from global memory (L1/L2 provide the reuse).  The field is accumulated
 // in the order H, x+, x-, y+, y-, z+, z- (DESIGN.md §3.1).
@@ -134,55 +180,21 @@ __global__ void __launch_bounds__(kThreads) sweep_generic_kernel(SweepArgs a, in
   const int q = rem % qpr; rem /= qpr;
   const int y = rem % L;
   const int z = rem / L;
-  const int c = colour, cc = 1 - colour;
+  const int c = colour;
   const int off = (y + z + c) & 1;
   const int j0 = q * V;
-  const int yp = (y + 1 == L) ? 0 : y + 1, ym = (y == 0) ? L - 1 : y - 1;
-  const int zp = (z + 1 == L) ? 0 : z + 1, zm = (z == 0) ? L - 1 : z - 1;
-  const int jx = off ? ((j0 + V == Lh) ? 0 : j0 + V) : ((j0 == 0) ? Lh - 1 : j0 - 1);   // the one x-neighbour outside [j0, j0+V)
-  const long long cs = comp_elems(g);
-
   float* S = a.spins + (long long)slot * 3 * g.N;
   const int d = slot / (g.O * g.T);
   const float* JH = a.jh + (long long)d * 6 * g.N;
 
-  // couplings: forward bonds of this site, backward bonds stored at the neighbour
-  const Vec<V> Jxp = ldv<V>(JH + jh_index(g, z, c, 0, y, j0));
-  const Vec<V> Jyp = ldv<V>(JH + jh_index(g, z, c, 1, y, j0));
-  const Vec<V> Jzp = ldv<V>(JH + jh_index(g, z, c, 2, y, j0));
-  const Vec<V> Jxq = ldv<V>(JH + jh_index(g, z, cc, 0, y, j0));
-  const float Jxe = JH[jh_index(g, z, cc, 0, y, jx)];
-  const Vec<V> Jym = ldv<V>(JH + jh_index(g, z, cc, 1, ym, j0));
-  const Vec<V> Jzm = ldv<V>(JH + jh_index(g, zm, cc, 2, y, j0));
-  Vec<V> Jxm;
-#pragma unroll
-  for (int e = 0; e < V; ++e) Jxm.v[e] = off ? Jxq.v[e] : (e > 0 ? Jxq.v[e > 0 ? e - 1 : 0] : Jxe);
-
   float h[3][V], own[3][V];
+  local_field_global<V>(g, S, JH, z, c, y, j0, h);
+  if (!HB) {
 #pragma unroll
-  for (int mu = 0; mu < 3; ++mu) {
-    const Vec<V> Hm = ldv<V>(JH + jh_index(g, z, c, 3 + mu, y, j0));
-    const Vec<V> sq = ldv<V>(S + spin_index(g, z, cc, mu, y, j0));
-    const float se = S[spin_index(g, z, cc, mu, y, jx)];
-    const Vec<V> syp = ldv<V>(S + spin_index(g, z, cc, mu, yp, j0));
-    const Vec<V> sym = ldv<V>(S + spin_index(g, z, cc, mu, ym, j0));
-    const Vec<V> szp = ldv<V>(S + spin_index(g, zp, cc, mu, y, j0));
-    const Vec<V> szm = ldv<V>(S + spin_index(g, zm, cc, mu, y, j0));
-    if (!HB) { const Vec<V> o = ldv<V>(S + spin_index(g, z, c, mu, y, j0));
+    for (int mu = 0; mu < 3; ++mu) {
+      const Vec<V> o = ldv<V>(S + spin_index(g, z, c, mu, y, j0));
 #pragma unroll
-      for (int e = 0; e < V; ++e) own[mu][e] = o.v[e]; }
-#pragma unroll
-    for (int e = 0; e < V; ++e) {
-      const float sxp = off ? (e + 1 < V ? sq.v[e + 1 < V ? e + 1 : 0] : se) : sq.v[e];
-      const float sxm = off ? sq.v[e] : (e > 0 ? sq.v[e > 0 ? e - 1 : 0] : se);
-      float acc = Hm.v[e];
-      acc = __fmaf_rn(Jxp.v[e], sxp, acc);
-      acc = __fmaf_rn(Jxm.v[e], sxm, acc);
-      acc = __fmaf_rn(Jyp.v[e], syp.v[e], acc);
-      acc = __fmaf_rn(Jym.v[e], sym.v[e], acc);
-      acc = __fmaf_rn(Jzp.v[e], szp.v[e], acc);
-      acc = __fmaf_rn(Jzm.v[e], szm.v[e], acc);
-      h[mu][e] = acc;
+      for (int e = 0; e < V; ++e) own[mu][e] = o.v[e];
     }
   }
 
@@ -247,10 +259,11 @@ __device__ __forceinline__ void block_reduce_store(double (&v)[NV], double* __re
 }
 
 // ------------------------------------------------------------------ energy (Eq. 1) and magnetisation per slot
-// One block per (slot, chunk of ZB planes); each thread takes items of V compact sites of one colour
-// (vector loads: own spins, the +x, +y, +z neighbours in the other colour's arrays, J and H), i.e. every
-// bond once.  partial[slot][chunk][4] = { -E contribution, sum s_x, sum s_y, sum s_z }.
-// Every fp32*fp32 product is exact in fp64; sums are fp64.
+// Eq. (1) in the bipartite form: every bond joins a colour-0 and a colour-1 site, so
+//   E = - sum_{i in colour 1} s_i . h_i  -  sum_{i in colour 0} s_i . H_i ,   h_i = the local field of §3.1 (H_i included).
+// Site terms in the spins' precision with the fixed FMA order of the moves, sums in fp64.
+// One block per (slot, chunk of ZB planes); each thread takes items of V compact sites of one colour.
+// partial[slot][chunk][4] = { -E contribution, sum s_x, sum s_y, sum s_z }.
 template <int V>
 __global__ void __launch_bounds__(kThreads) energy_mag_kernel(Geom g, int ZB, const float* __restrict__ spins, const float* __restrict__ jh,
                                                               double* __restrict__ partial) {
@@ -266,43 +279,28 @@ __global__ void __launch_bounds__(kThreads) energy_mag_kernel(Geom g, int ZB, co
     const int q = it % qpr; int rem = it / qpr;
     const int y = rem % L; rem /= L;
     const int c = rem & 1; const int z = z0 + (rem >> 1);
-    const int cc = 1 - c, j0 = q * V;
-    const int off = (y + z + c) & 1;
-    const int yp = (y + 1 == L) ? 0 : y + 1, zp = (z + 1 == L) ? 0 : z + 1;
-    const int je = (j0 + V == Lh) ? 0 : j0 + V;     // +x neighbour outside the vector (used when off = 1)
-    const Vec<V> Jx = ldv<V>(JH + jh_index(g, z, c, 0, y, j0));
-    const Vec<V> Jy = ldv<V>(JH + jh_index(g, z, c, 1, y, j0));
-    const Vec<V> Jz = ldv<V>(JH + jh_index(g, z, c, 2, y, j0));
-    double dx[V], dy[V], dz[V], hs[V];
+    const int j0 = q * V;
+    float h[3][V], s[3][V];
+    if (c == 1) {
+      local_field_global<V>(g, S, JH, z, c, y, j0, h);
+    } else {
 #pragma unroll
-    for (int e = 0; e < V; ++e) { dx[e] = 0.0; dy[e] = 0.0; dz[e] = 0.0; hs[e] = 0.0; }
+      for (int mu = 0; mu < 3; ++mu) {
+        const Vec<V> Hm = ldv<V>(JH + jh_index(g, z, c, 3 + mu, y, j0));
+#pragma unroll
+        for (int e = 0; e < V; ++e) h[mu][e] = Hm.v[e];
+      }
+    }
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) {
-      const Vec<V> s = ldv<V>(S + spin_index(g, z, c, mu, y, j0));
-      const Vec<V> sx = ldv<V>(S + spin_index(g, z, cc, mu, y, j0));
-      const float se = off ? S[spin_index(g, z, cc, mu, y, je)] : 0.0f;
-      const Vec<V> sy = ldv<V>(S + spin_index(g, z, cc, mu, yp, j0));
-      const Vec<V> sz = ldv<V>(S + spin_index(g, zp, cc, mu, y, j0));
-      const Vec<V> Hm = ldv<V>(JH + jh_index(g, z, c, 3 + mu, y, j0));
-      double msum = 0.0;
+      const Vec<V> sv = ldv<V>(S + spin_index(g, z, c, mu, y, j0));
 #pragma unroll
-      for (int e = 0; e < V; ++e) {
-        const double sd = (double)s.v[e];
-        const float xn = off ? (e + 1 < V ? sx.v[e + 1 < V ? e + 1 : 0] : se) : sx.v[e];
-        dx[e] = fma(sd, (double)xn, dx[e]);
-        dy[e] = fma(sd, (double)sy.v[e], dy[e]);
-        dz[e] = fma(sd, (double)sz.v[e], dz[e]);
-        hs[e] = fma((double)Hm.v[e], sd, hs[e]);
-        msum += sd;
-      }
-      acc[1 + mu] += msum;
+      for (int e = 0; e < V; ++e) { s[mu][e] = sv.v[e]; acc[1 + mu] += (double)sv.v[e]; }
     }
 #pragma unroll
     for (int e = 0; e < V; ++e) {
-      double en = (double)Jx.v[e] * dx[e];
-      en = fma((double)Jy.v[e], dy[e], en);
-      en = fma((double)Jz.v[e], dz[e], en);
-      acc[0] += en + hs[e];
+      const Vec3 sv = {s[0][e], s[1][e], s[2][e]}, hv = {h[0][e], h[1][e], h[2][e]};
+      acc[0] += (double)dot3(sv, hv);
     }
   }
   block_reduce_store<4>(acc, partial + (long long)blockIdx.x * 4);

@@ -245,7 +245,7 @@ struct Th {
 struct HbPar { float beta; uint32_t sysid, c1, c3; PhiloxKey key; };
 
 // fp64 partial sums of one thread in the final sweep of a call:
-// e = sum_{i in colour 1} s_i.(sum_6 J_ij s_j) + sum_i H_i.s_i  (= -E), m = sum_i s_i; exact fp32 x fp32 products
+// e = sum_{i in colour 1} s_i.h_i + sum_{i in colour 0} s_i.H_i  (= -E, site terms in fp32: DESIGN.md §3.6), m = sum_i s_i
 struct EAcc { double e, mx, my, mz; };
 
 // shared-memory addresses of the coupling / field arrays one colour update reads
@@ -262,9 +262,9 @@ struct JAddr {
 // `xs` = shared-memory half-plane of the other colour in this plane (rows y+-1 and the x edge),
 // `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1.  CSB / CJB = byte strides between the
 // component arrays of a shared spin half-plane / between the arrays of a shared J/H plane.
-// EN = 0: move only; 1: also accumulate H_i.s_i and s_i of the NEW spin (colour 0 in the final sweep);
-// 2: additionally s_i.(sum_6 J_ij s_j) with every bond of the site (colour 1 in the final sweep, when all its
-// neighbours already hold their final values).
+// EN = 0: move only; 1: also accumulate s_i.H_i and s_i of the NEW spin (colour 0 in the final sweep);
+// 2: s_i.h_i instead, the whole local field (colour 1 in the final sweep, when all its neighbours already hold their
+// final values: every bond of the lattice once).
 template <uint32_t CSB, uint32_t CJB, int V, bool HB, int EN>
 __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&own)[3][V], const float (&q)[3][V],
                                              const float (&zlo)[3][V], const float (&zhi)[3][V], uint32_t xs,
@@ -285,7 +285,6 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
   lds<V>(Jzm, ja.oth_z + th.row);
   float h[3][V];
   float Hs[3][V];
-  double hd[3][V];
   const uint32_t xs_p = xs + th.rowp, xs_m = xs + th.rowm, xs_e = xs + edge;
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
@@ -306,16 +305,7 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
       acc = __fmaf_rn(Jzp[e], zhi[mu][e], acc);
       acc = __fmaf_rn(Jzm[e], zlo[mu][e], acc);
       h[mu][e] = acc;
-      if (EN >= 1) Hs[mu][e] = Hm[e];
-      if (EN == 2) {
-        double d = (double)Jxp[e] * (double)sxp;
-        d = fma((double)Jxm[e], (double)sxm, d);
-        d = fma((double)Jyp[e], (double)yp[e], d);
-        d = fma((double)Jym[e], (double)ym[e], d);
-        d = fma((double)Jzp[e], (double)zhi[mu][e], d);
-        d = fma((double)Jzm[e], (double)zlo[mu][e], d);
-        hd[mu][e] = d;
-      }
+      if (EN == 1) Hs[mu][e] = Hm[e];
     }
   }
   // heat bath: one Philox call per pair of sites (e, e+1), e even: counter word 0 = the site with even compact index
@@ -338,16 +328,9 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
     }
     out[0][e] = s.x; out[1][e] = s.y; out[2][e] = s.z;
     if (EN >= 1) {
-      const double sx = (double)s.x, sy = (double)s.y, sz = (double)s.z;
-      double d = (double)Hs[0][e] * sx;
-      d = fma((double)Hs[1][e], sy, d);
-      d = fma((double)Hs[2][e], sz, d);
-      if (EN == 2) {
-        d = fma(hd[0][e], sx, d);
-        d = fma(hd[1][e], sy, d);
-        d = fma(hd[2][e], sz, d);
-      }
-      ea.e += d; ea.mx += sx; ea.my += sy; ea.mz += sz;
+      const Vec3 f = {EN == 2 ? h[0][e] : Hs[0][e], EN == 2 ? h[1][e] : Hs[1][e], EN == 2 ? h[2][e] : Hs[2][e]};
+      ea.e += (double)dot3(s, f);
+      ea.mx += (double)s.x; ea.my += (double)s.y; ea.mz += (double)s.z;
     }
   }
 }

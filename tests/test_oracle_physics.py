@@ -56,6 +56,16 @@ def test_energy_matches_three_algebraically_equal_forms():
     # zero field path (H = None)
     sim.set_disorder(J, None)
     assert abs(sim.energy()[0, 0, 0] - energy_roll(S[0, 0, 0].astype(np.float64), J[0].astype(np.float64), None)) < 1e-11
+    # fp32 instantiation: the site terms s_i.h_i (odd sites) and s_i.H_i (even sites) are single-precision FMA chains
+    # (spins single, aggregates double), summed in double.  Each odd-site term carries at most
+    # 9 roundings of 2^-24 relative to sum|J||s||s| + |H||s| <~ 8: |E32 - E| <= N/2 * 9 * 2^-24 * 8; typically sqrt(N) smaller.
+    sim32 = oracle.Oracle(L, D, O, temps, 1, precision=32)
+    sim32.set_disorder(J, H); sim32.set_spins(S)
+    E32 = sim32.energy()
+    N = L**3
+    assert np.abs(E32 - E).max() < N / 2 * 9 * 2.0**-24 * 8
+    assert np.abs(E32 - E).max() < 40 * math.sqrt(N) * 2.0**-24 * 8       # random-walk size, with margin
+    assert np.abs(E32 - E).max() > 0                                      # it IS the single-precision form
 
 
 # ---------------------------------------------------------------------- OR sweeps are microcanonical
@@ -144,7 +154,8 @@ def test_dimers_zero_field_closed_form(J0, T):
     assert abs(acc.mean() - exact) < 4.5 * err + 1e-5
     # the energy routine sees the same number: E = -J0 * sum over dimers of s1.s2
     S = sim.get_spins()[0, 0, 0]
-    assert abs(sim.energy()[0, 0, 0] + float(np.float32(J0)) * (S[:, :, :, 0::2] * S[:, :, :, 1::2]).sum()) < 1e-9
+    # (fp32 instantiation: site terms s_i.h_i are single-precision FMA chains, DESIGN.md §3.6 -> a few 2^-24 per site)
+    assert abs(sim.energy()[0, 0, 0] + float(np.float32(J0)) * (S[:, :, :, 0::2] * S[:, :, :, 1::2]).sum()) < 2e-7 * L**3
 
 
 def _dimer_in_field_exact(beta, J0, h1, h2):
