@@ -80,11 +80,12 @@ namespace zm {
 #endif
 constexpr int kUnroll = HSG_ZM_UNROLL;   // unroll factor of the main march loop
 constexpr int kUnrollHB = HSG_ZM_UNROLL_HB;
-constexpr int kDS = HSG_ZM_DS, kDJ = HSG_ZM_DJ;
-constexpr int kNC1 = kDS + 2;            // ring C1: planes k, k+1 live + DS in flight
-constexpr int kNC0 = kDS + 1;            // ring C0: plane k live + DS in flight
-constexpr int kNJA = kDJ + 2;            // J/H ring A: planes k-1, k live + DJ in flight
-constexpr int kNJB = kDJ + 3;            // J/H ring B: planes k-2, k-1, k live + DJ in flight; also the mbarrier ring
+#ifndef HSG_ZM_L64_DS
+#define HSG_ZM_L64_DS 2          // (3 with DJ = 1 fits too and gains 1 % on c5; DJ = 1 is not validated for G = 1)
+#endif
+#ifndef HSG_ZM_L64_DJ
+#define HSG_ZM_L64_DJ 2
+#endif
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -209,22 +210,29 @@ template <int L, int YS, int V, int G> struct Cfg {
   static constexpr int HPS = 3 * CSS;
   static constexpr int CSJ = (YS + (HALO ? 1 : 0)) * Lh;   // shared J/H array: halo row below (for the -y couplings), YS rows
   static constexpr int JA = 11 * CSJ;             // ring A slot: 11 arrays; ring B slot: colour-0 Jz
-  static constexpr int NJA = kNJA, NJB = kNJB;    // J/H ring depths (ring_advance)
+  static constexpr int DS = L == 64 ? HSG_ZM_L64_DS : HSG_ZM_DS;   // spin planes in flight ahead of the step that uses them
+  static constexpr int DJ = L == 64 ? HSG_ZM_L64_DJ : HSG_ZM_DJ;   // J/H planes in flight
+  static constexpr int NC1 = DS + 2;              // ring C1: planes k, k+1 live + DS in flight
+  static constexpr int NC0 = DS + 1;              // ring C0: plane k live + DS in flight
+  static constexpr int NJA = DJ + 2;              // J/H ring A: planes k-1, k live + DJ in flight
+  static constexpr int NJB = DJ + 3;              // J/H ring B: planes k-2, k-1, k live + DJ in flight; also the mbarrier ring
+  static constexpr int CS0 = YS * Lh;             // ring C0 holds own columns only: no halo rows
+  static constexpr int HP0 = 3 * CS0;
   static constexpr int RW = TPS < 32 ? TPS : 32;  // shuffle width of the per-system reduction
   static constexpr int WPS = TPS / RW;            // partial sums per system after the shuffle stage
   // byte offsets inside dynamic shared memory
-  static constexpr uint32_t red_off = 64;         // [G][WPS][4] doubles (after kNJB <= 6 J/H mbarriers and 2 halo mbarriers)
+  static constexpr uint32_t red_off = 64;         // [G][WPS][4] doubles (after NJB <= 6 J/H mbarriers and 2 halo mbarriers)
   static constexpr uint32_t red2_off = red_off + G * WPS * 32;        // [G][NCL][4] doubles: per-strip sums, used in rank 0
   static constexpr uint32_t ja_off = 128 * ((red2_off + G * NCL * 32 + 127) / 128);
-  static constexpr uint32_t jb_off = ja_off + 4u * kNJA * JA;
-  static constexpr uint32_t sys_off = jb_off + 4u * kNJB * CSJ;
-  static constexpr uint32_t sys_bytes = 4u * (kNC1 + kNC0 + 2) * HPS;    // per system: C1 ring, C0 ring, X0[2]
+  static constexpr uint32_t jb_off = ja_off + 4u * NJA * JA;
+  static constexpr uint32_t sys_off = jb_off + 4u * NJB * CSJ;
+  static constexpr uint32_t sys_bytes = 4u * ((NC1 + 2) * HPS + NC0 * HP0);    // per system: C1 ring, X0[2], C0 ring
   static constexpr size_t smem_bytes = sys_off + (size_t)G * sys_bytes;
   static_assert(L % YS == 0 && Lh % V == 0 && V % 2 == 0, "strip height divides L, even vector width divides the row length");
   static_assert((YS * Lh * 4) % 16 == 0 && (Lh * 4) % 16 == 0, "bulk copies move multiples of 16 bytes");
   static_assert(!HALO || V == 4, "halo copies use 16-byte cp.async.cg");
   static_assert(!HALO || YS >= 2, "a thread is on at most one strip edge");
-  static_assert(kNJB <= 6, "mbarrier area holds kNJB J/H barriers and two halo barriers");
+  static_assert(NJB <= 6, "mbarrier area holds NJB J/H barriers and two halo barriers");
   static constexpr uint32_t halo_bytes = G * 2u * 3u * Lh * 4u;   // new colour-0 halo rows received per step: both neighbours, G systems
   static_assert(smem_bytes <= 232448, "exceeds the 227 KB of shared memory per CTA");
 };
@@ -236,6 +244,7 @@ struct Th {
   int grow_halo;              // HALO edge threads: element offset of the halo row they fetch (row gy-1 or gy+1, periodic)
   int edge;                   // HALO: -1 = lowest row of the strip, +1 = highest row, 0 = interior
   uint32_t row, rowp, rowm;   // byte offsets inside a shared [y][j] array: own row, row y+1, row y-1 at j0
+  uint32_t row0;              // own row at j0 inside an array without halo rows (ring C0)
   uint32_t edge0, edge1;      // own row at j0-1 and j0+V (periodic): the x neighbour outside the thread's V sites
   uint32_t halo;              // HALO edge threads: byte offset of the halo row they fill (== rowm or rowp)
   uint32_t push;              // HALO edge threads: cluster address of X0[0], component 0, halo row at j0 in the neighbour CTA
@@ -337,9 +346,9 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
 
 // Shared state of one CTA during the march (32-bit shared-window addresses)
 struct Smem {
-  uint32_t full;       // [kNJB] mbarriers of the J/H stream
+  uint32_t full;       // [NJB] mbarriers of the J/H stream
   uint32_t hfull;      // [2] mbarriers: halo rows of X0[0], X0[1] have arrived from the neighbour strips
-  uint32_t ja, jb;     // J/H rings A ([kNJA][11 CSJ]) and B ([kNJB][CSJ])
+  uint32_t ja, jb;     // J/H rings A ([NJA][11 CSJ]) and B ([NJB][CSJ])
   uint32_t c1, c0;     // this thread's system: rings of old colour-1 / colour-0 half-planes
   uint32_t x0;         // this thread's system: [2][HPS] new colour-0 spins of planes k-1, k
   int y0;              // first row of this CTA's strip
@@ -349,7 +358,7 @@ struct Stream {        // J/H plane stream: index q -> plane (q-1) mod L
   int issued, waited, total;
 };
 
-// J/H stream: warp 0 keeps kDJ planes in flight beyond the newest index `nd` this step reads; everyone waits for nd.
+// J/H stream: warp 0 keeps DJ planes in flight beyond the newest index `nd` this step reads; everyone waits for nd.
 // Slot reuse is safe because the barrier that ended the previous step separates the last reads of index
 // nd-2 (ring A) and nd-3 (ring B) from the copies issued here.  Whole-plane CTAs move a plane with two bulk copies;
 // strip CTAs move the YS rows of each of the twelve arrays plus the halo row of the two Jy arrays (14 copies, one per lane).
@@ -357,7 +366,7 @@ template <class C, int L, class SmemT>
 __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __restrict__ jh_d, Stream& st, int nd, uint64_t pol) {
   constexpr uint32_t JAB = 4u * C::JA, JBB = 4u * C::CSJ;
   if (threadIdx.x < 32) {
-    const int upto = min(nd + kDJ, st.total - 1);
+    const int upto = min(nd + C::DJ, st.total - 1);
     while (st.issued < upto) {
       ++st.issued;
       const int plane = (st.issued + L - 1) % L;
@@ -432,6 +441,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   using C = Cfg<L, YS, V, G>;
   constexpr int CS = C::CSG, HP = C::HPG, PS = 2 * C::HPG;
   constexpr uint32_t CSB = 4u * C::CSS, HPB = 4u * C::HPS, CJB = 4u * C::CSJ, JAB = 4u * C::JA, JBB = 4u * C::CSJ;
+  constexpr uint32_t CS0B = 4u * C::CS0, HP0B = 4u * C::HP0;
   constexpr bool HALO = C::HALO;
   float A[3][V], B[3][V], Cc[3][V], O[3][V], P[3][V], Q[3][V], R[3][V], On[3][V];
   float* Sr = S + th.grow;                             // own column, plane 0, colour 0, component 0
@@ -446,15 +456,15 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
       if (HALO && th.edge != 0) cp_async<V>(d1 + mu * CSB + th.halo, Sh + zc * PS + HP + mu * CS, pol_spin);
     }
   };
-  // stage t = the planes step t consumes for the first time: old colour 1 of plane t+1 (ring C1, slot (t+1) % kNC1)
-  // and, for over-relaxation, old colour 0 of plane t (ring C0, slot t % kNC0); own column only.
+  // stage t = the planes step t consumes for the first time: old colour 1 of plane t+1 (ring C1, slot (t+1) % C::NC1)
+  // and, for over-relaxation, old colour 0 of plane t (ring C0, slot t % C::NC0); own column only.
   auto issue_stage = [&](int t) {
     if (t < L) {
-      fetch_c1((t + 1 == L) ? 0 : t + 1, (t + 1) % kNC1);
+      fetch_c1((t + 1 == L) ? 0 : t + 1, (t + 1) % C::NC1);
       if (!HB) {
-        const uint32_t d0 = sm.c0 + (uint32_t)(t % kNC0) * HPB + th.row;
+        const uint32_t d0 = sm.c0 + (uint32_t)(t % C::NC0) * HP0B + th.row0;
 #pragma unroll
-        for (int mu = 0; mu < 3; ++mu) cp_async<V>(d0 + mu * CSB, Sr + t * PS + mu * CS, pol_spin);
+        for (int mu = 0; mu < 3; ++mu) cp_async<V>(d0 + mu * CS0B, Sr + t * PS + mu * CS, pol_spin);
       }
     }
     cp_async_commit();                                  // an empty group keeps the group count uniform
@@ -482,14 +492,14 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   fetch_c1(0, 0);
   cp_async_commit();
 #pragma unroll
-  for (int t = 0; t < kDS; ++t) issue_stage(t);
+  for (int t = 0; t < C::DS; ++t) issue_stage(t);
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
     ldg<V>(A[mu], Sr + (L - 1) * PS + HP + mu * CS);
 #pragma unroll
     for (int e = 0; e < V; ++e) { P[mu][e] = 0.0f; Q[mu][e] = 0.0f; O[mu][e] = 0.0f; On[mu][e] = 0.0f; }
   }
-  cp_async_wait<kDS>();
+  cp_async_wait<C::DS>();
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) lds<V>(B[mu], sm.c1 + mu * CSB + th.row);
   step_end<C>();
@@ -499,27 +509,27 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     const int nd = qbase + k + 1;                       // newest J/H stream index this step reads (plane k)
     ring_advance<C, L>(sm, jh_d, st, nd, pol_jh);
     arm_halo((uint32_t)(k & 1));
-    cp_async_wait<kDS - 1>();                           // stage k has landed (own column)
+    cp_async_wait<C::DS - 1>();                           // stage k has landed (own column)
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) {
-      lds<V>(Cc[mu], sm.c1 + (uint32_t)((k + 1) % kNC1) * HPB + mu * CSB + th.row);
-      if (!HB) lds<V>(O[mu], sm.c0 + (uint32_t)(k % kNC0) * HPB + mu * CSB + th.row);
+      lds<V>(Cc[mu], sm.c1 + (uint32_t)((k + 1) % C::NC1) * HPB + mu * CSB + th.row);
+      if (!HB) lds<V>(O[mu], sm.c0 + (uint32_t)(k % C::NC0) * HP0B + mu * CS0B + th.row0);
     }
-    issue_stage(k + kDS);
+    issue_stage(k + C::DS);
     if (k + 1 == L) {                                   // the new colour 0 of plane 0, needed by step L
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) ldg<V>(On[mu], Sr + mu * CS);
     }
     const int off = (th.gy + k) & 1;
-    const uint32_t ak = sm.ja + ((uint32_t)nd % kNJA) * JAB;                     // plane k
-    const uint32_t ak1 = sm.ja + ((uint32_t)(nd + kNJA - 1) % kNJA) * JAB;       // plane k-1
-    const uint32_t bk = sm.jb + ((uint32_t)nd % kNJB) * JBB;                     // colour-0 Jz of plane k
-    const uint32_t bk2 = sm.jb + ((uint32_t)(nd + kNJB - 2) % kNJB) * JBB;       // colour-0 Jz of plane k-2
+    const uint32_t ak = sm.ja + ((uint32_t)nd % C::NJA) * JAB;                     // plane k
+    const uint32_t ak1 = sm.ja + ((uint32_t)(nd + C::NJA - 1) % C::NJA) * JAB;       // plane k-1
+    const uint32_t bk = sm.jb + ((uint32_t)nd % C::NJB) * JBB;                     // colour-0 Jz of plane k
+    const uint32_t bk2 = sm.jb + ((uint32_t)(nd + C::NJB - 2) % C::NJB) * JBB;       // colour-0 Jz of plane k-2
     const uint32_t par = (uint32_t)(k & 1);
     {
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * k));
       const JAddr ja = {ak, bk, ak + 2 * CJB, ak + 5 * CJB, ak1 + 7 * CJB};
-      update_sites<CSB, CJB, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % kNC1) * HPB, ja, th, off, hp, site0, ea);
+      update_sites<CSB, CJB, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % C::NC1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + k * PS + mu * CS, R[mu]);
       step_wait<C>();
@@ -561,8 +571,8 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     }
     wait_halo((uint32_t)((k - 1) & 1));
     const int off = (th.gy + k) & 1;
-    const uint32_t a1 = sm.ja + ((uint32_t)nd % kNJA) * JAB;                     // plane k-1
-    const uint32_t b2 = sm.jb + ((uint32_t)(nd + kNJB - 1) % kNJB) * JBB;        // colour-0 Jz of plane k-2
+    const uint32_t a1 = sm.ja + ((uint32_t)nd % C::NJA) * JAB;                     // plane k-1
+    const uint32_t b2 = sm.jb + ((uint32_t)(nd + C::NJB - 1) % C::NJB) * JBB;        // colour-0 Jz of plane k-2
     const int z1 = kk == 0 ? L - 1 : 0;
     const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * z1));
     const JAddr ja = {a1 + 5 * CJB, a1 + 7 * CJB, a1 + 8 * CJB, a1, b2};
@@ -593,12 +603,12 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
   sm.ja = base + C::ja_off;
   sm.jb = base + C::jb_off;
   sm.c1 = base + C::sys_off + (uint32_t)gs * C::sys_bytes;
-  sm.c0 = sm.c1 + 4u * kNC1 * C::HPS;
-  sm.x0 = sm.c0 + 4u * kNC0 * C::HPS;
+  sm.x0 = sm.c1 + 4u * C::NC1 * C::HPS;
+  sm.c0 = sm.x0 + 4u * 2 * C::HPS;
   sm.y0 = rank * YS;
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int i = 0; i < kNJB; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
+    for (int i = 0; i < C::NJB; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + 6, 1);
     mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + 7, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -612,6 +622,7 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
   th.gy = sm.y0 + ly;
   th.grow = th.gy * C::Lh + th.j0;
   th.row = 4u * (uint32_t)((ly + HR) * C::Lh + th.j0);
+  th.row0 = 4u * (uint32_t)(ly * C::Lh + th.j0);
   if (C::HALO) {
     th.rowp = th.row + 4u * C::Lh;
     th.rowm = th.row - 4u * C::Lh;
