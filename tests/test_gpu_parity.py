@@ -265,3 +265,44 @@ def test_energy_fused_into_the_last_sweep_matches_oracle_and_the_separate_reduct
     eng2.init_spins(); eng2.sweep(n_or, n_hb)
     np.testing.assert_allclose(eng2.energy().cpu().numpy(), E, rtol=1e-13)
     assert np.array_equal(eng2.get_spins().cpu().numpy(), eng.get_spins().cpu().numpy())
+
+
+@pytest.mark.parametrize("cfg,samples", [("c2", (0, 101, 255)), ("c3", (7, 200)), ("c4", (0, 37, 63)), ("c5", (5,))])
+def test_full_size_configs_on_sampled_disorder_samples(cfg, samples):
+    """BASELINE.json's full sizes, in the launch configuration bench.py times (all samples resident, the sweep kernel
+    bench.py uses): two steps of (4 OR + 1 HB) + PT + measure.  The oracle recomputes individual disorder samples — every
+    sample has its own input stream and its own Philox system ids, so one sample of the full run is a run of its own —
+    and every spin, swap decision and observable of those samples must agree (spins to the bit)."""
+    import paper_1204_6192_b200 as hsg
+    c, temps, J, H = hsg_inputs.make_config(cfg)
+    L, D, O, T = c["L"], c["n_samples"], c["n_replicas"], len(temps)
+    eng = hsg.hsg_create(L, D, O, temps, c["seed"])
+    eng.set_disorder(J, H); eng.init_spins()
+    accs = []
+    for _ in range(2):
+        eng.sweep(4, 1)
+        accs.append(eng.pt_swap().cpu().numpy())
+    assert eng.last_sweep_kernel() == "zmarch"
+    E, M, q0, qk = (x.cpu().numpy() for x in eng.measure())
+    S = eng.get_spins()
+    N = L ** 3
+    for d in samples:
+        orc = oracle.Oracle(L, 1, O, temps, c["seed"], precision=32, sample_offset=d, n_threads=8)
+        orc.set_disorder(J[d:d + 1], None if H is None else H[d:d + 1]); orc.init_spins()
+        for k in range(2):
+            orc.sweep(4, 1)
+            assert np.array_equal(orc.pt_swap()[0], accs[k][d]), f"{cfg} sample {d}: swap decisions of step {k}"
+        a = S[d].cpu().numpy().astype(np.float64)
+        b = orc.get_spins()[0]
+        assert np.abs(a - b).max() == 0.0, f"{cfg} sample {d}: spins"
+        Eo, Mo, q0o, qko = orc.measure()
+        np.testing.assert_allclose(E[d], np.asarray(Eo)[0], rtol=1e-12)
+        assert np.abs(E[d] / np.asarray(Eo)[0] - 1).max() <= 1e-5
+        np.testing.assert_allclose(M[d], np.asarray(Mo).reshape(M[d].shape), rtol=0, atol=1e-13)
+        np.testing.assert_allclose(q0[d], np.asarray(q0o).reshape(q0[d].shape), rtol=0, atol=1e-12)
+        np.testing.assert_allclose(qk[d], np.asarray(qko).reshape(qk[d].shape), rtol=0, atol=1e-12)
+    # properties that hold for every system of the full run: unit spins, permutation intact
+    nrm = (S.reshape(D * O * T, 3, N) ** 2).sum(dim=1)
+    assert float((nrm - 1).abs().max()) < 1e-4
+    perm, cnt = eng.get_state()
+    assert (np.sort(np.asarray(perm.cpu() if hasattr(perm, "cpu") else perm), axis=2) == np.arange(T)).all() and tuple(cnt) == (2, 2)
