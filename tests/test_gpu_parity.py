@@ -306,3 +306,40 @@ def test_full_size_configs_on_sampled_disorder_samples(cfg, samples):
     assert float((nrm - 1).abs().max()) < 1e-4
     perm, cnt = eng.get_state()
     assert (np.sort(np.asarray(perm.cpu() if hasattr(perm, "cpu") else perm), axis=2) == np.arange(T)).all() and tuple(cnt) == (2, 2)
+
+
+def test_equilibrium_energy_and_q2_agree_over_64_samples():
+    """BASELINE.json: equilibrium energy and q^2 agreeing within 3 sigma over 64 samples.  L = 8, 64 samples x 2 replicas
+    x 8 temperatures, 5 OR + 1 HB + PT per step.  (i) Same Philox seed: the free-running GPU and oracle chains stay
+    identical, so the averages coincide.  (ii) An independent GPU chain (another Philox seed, the same disorder): the
+    per-sample paired differences of <e> and <q^2> average to zero within 3 sigma of their spread over the 64 samples."""
+    import paper_1204_6192_b200 as hsg
+    L, D, O, T, dseed = 8, 64, 2, 8, 21
+    temps = hsg_inputs.geometric_ladder(0.12, 0.40, T)
+    J = hsg_inputs.couplings(L, D, dseed); H = hsg_inputs.gaussian_field(L, D, 0.1, dseed)
+    n_eq, n_meas, N = 60, 60, L ** 3
+
+    def run(sim, is_gpu):
+        sim.set_disorder(J, H); sim.init_spins()
+        e_acc = np.zeros((D, O, T)); q_acc = np.zeros((D, T))
+        for step in range(n_eq + n_meas):
+            sim.sweep(5, 1); sim.pt_swap()
+            if step >= n_eq:
+                E, _, q0, _ = sim.measure()
+                if is_gpu:
+                    E, q0 = E.cpu().numpy(), q0.cpu().numpy()
+                e_acc += np.asarray(E).reshape(D, O, T) / N
+                q_acc += (np.asarray(q0).reshape(D, T, 9) ** 2).sum(axis=2)
+        return e_acc.mean(axis=1) / n_meas, q_acc / n_meas            # [D][T] each
+
+    e_o, q_o = run(oracle.Oracle(L, D, O, temps, 1001, precision=32, n_threads=16), False)
+    e_g, q_g = run(hsg.hsg_create(L, D, O, temps, 1001), True)
+    np.testing.assert_allclose(e_g, e_o, rtol=1e-11)                  # identical chains
+    np.testing.assert_allclose(q_g, q_o, rtol=0, atol=1e-11)
+    e_i, q_i = run(hsg.hsg_create(L, D, O, temps, 2002), True)        # independent chain
+    for name, a, b in (("e", e_i, e_o), ("q2", q_i, q_o)):
+        diff = a - b                                                  # [D][T], paired by disorder sample
+        mean, sem = diff.mean(axis=0), diff.std(axis=0, ddof=1) / np.sqrt(D)
+        assert (np.abs(mean) < 3.0 * sem + 1e-12).sum() >= T - 1, (name, mean / sem)   # 3 sigma at (at least) 7 of 8 temperatures
+        assert np.abs(mean / sem).max() < 4.5, (name, mean / sem)
+    assert (e_o[:, 0] < e_o[:, -1]).all() and (q_o[:, 0].mean() > q_o[:, -1].mean())   # colder: lower energy, larger overlap
