@@ -104,11 +104,11 @@ def _dist():
 
 
 # ------------------------------------------------------------------------------------------------ oracle arms
-def run_oracle(cfg, temps, steps, warmup, n_systems_cap=64):
+def run_oracle(cfg, temps, steps, warmup, n_systems_cap=64, threads=None, precision=32):
     """Time the oracle as it stands on a bounded sample of the workload: the first sample's systems
     (at most n_systems_cap of them), `steps` full steps after `warmup`.  Returns (ns/update, cores, text)."""
     import oracle
-    cores = os.cpu_count() or 1
+    cores = threads or os.cpu_count() or 1
     O = cfg["n_replicas"]
     T = len(temps)
     while O * T > n_systems_cap and T > 2:
@@ -117,7 +117,7 @@ def run_oracle(cfg, temps, steps, warmup, n_systems_cap=64):
     L = cfg["L"]
     J = hsg_inputs.couplings(L, 1, cfg["seed"])
     H = hsg_inputs.gaussian_field(L, 1, cfg["h_r"], cfg["seed"]) if cfg["h_r"] > 0 else None
-    sim = oracle.Oracle(L, 1, O, tsub, cfg["seed"], precision=32, n_threads=cores)
+    sim = oracle.Oracle(L, 1, O, tsub, cfg["seed"], precision=precision, n_threads=cores)
     sim.set_disorder(J, H); sim.init_spins()
     def step():
         sim.sweep(cfg["n_or"], cfg["n_hb"]); sim.pt_swap(); sim.measure()
@@ -129,7 +129,7 @@ def run_oracle(cfg, temps, steps, warmup, n_systems_cap=64):
     dt = time.perf_counter() - t0
     updates = (cfg["n_or"] + cfg["n_hb"]) * O * T * L ** 3 * steps
     text = (f"{steps} steps ({cfg['n_or']} OR + {cfg['n_hb']} HB + PT + measure) of 1 sample x {O} replicas x {T} temperatures, "
-            f"L={L}, fp32 oracle, {cores} threads over systems")
+            f"L={L}, fp{precision} oracle, {cores} threads over systems")
     return dt / updates * 1e9, cores, text, dt / steps * 1e3
 
 
@@ -137,7 +137,8 @@ def main_reference(args, cfg, temps):
     rank, world, _ = _dist()
     if rank != 0:
         return
-    ns, cores, text, ms = run_oracle(cfg, temps, max(1, args.steps), max(0, min(args.warmup, 1)))
+    ns, cores, text, ms = run_oracle(cfg, temps, max(1, args.steps), max(0, min(args.warmup, 1)),
+                                     n_systems_cap=args.cpu_systems, threads=args.cpu_threads, precision=args.cpu_precision)
     line = {"impl": "reference", "metric": METRIC, "value": ns, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic", "config": {"workload": args.workload, "note": "oracle on host cores, bounded sample"},
@@ -345,6 +346,9 @@ def main():
     ap.add_argument("--no-measure", action="store_true")
     ap.add_argument("--no-fuse-energy", action="store_true", help="separate energy reduction kernel instead of the fused final sweep")
     ap.add_argument("--cpu-steps", type=int, default=3, help="oracle steps timed for cpu_baseline")
+    ap.add_argument("--cpu-threads", type=int, default=None, help="--impl reference: oracle threads (default: all host cores)")
+    ap.add_argument("--cpu-systems", type=int, default=64, help="--impl reference: systems in the bounded sample")
+    ap.add_argument("--cpu-precision", type=int, default=32, choices=[32, 64], help="--impl reference: oracle instantiation")
     args = ap.parse_args()
     cfg = dict(hsg_inputs.CONFIGS[args.workload])
     if args.samples is not None:
