@@ -70,6 +70,7 @@ int check_desc(const hsg_desc* d) {
 Geom make_geom(const hsg_desc* d) {
   Geom g{};
   g.L = d->L; g.Lh = d->L / 2;
+  g.ys = d->L == 64 ? 16 : d->L;           // strips of the J/H layout (hsg_layout.cuh) = strips of zmarch_kernel<64,16,..>
   g.D = d->n_samples; g.O = d->n_replicas; g.T = d->n_temps;
   g.R = g.D * g.O * g.T;
   g.N = (long long)d->L * d->L * d->L;

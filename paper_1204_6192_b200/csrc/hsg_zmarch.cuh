@@ -208,8 +208,9 @@ template <int L, int YS, int V, int G> struct Cfg {
   static constexpr int HPG = 3 * CSG;             // spin half-plane (one colour, 3 components) in global memory
   static constexpr int CSS = (YS + (HALO ? 2 : 0)) * Lh;   // shared spin array: halo row below, YS rows, halo row above
   static constexpr int HPS = 3 * CSS;
-  static constexpr int CSJ = (YS + (HALO ? 1 : 0)) * Lh;   // shared J/H array: halo row below (for the -y couplings), YS rows
-  static constexpr int JA = 11 * CSJ;             // ring A slot: 11 arrays; ring B slot: colour-0 Jz
+  static constexpr int CSJ = YS * Lh;             // shared J/H array of a strip
+  static constexpr int JA = 11 * CSJ + (HALO ? 2 * Lh : 0);   // ring A slot: 11 arrays, then (strips) the row y0-1 of the two Jy
+                                                              // arrays (colour 0, colour 1); ring B slot: colour-0 Jz
   static constexpr int DS = L == 64 ? HSG_ZM_L64_DS : HSG_ZM_DS;   // spin planes in flight ahead of the step that uses them
   static constexpr int DJ = L == 64 ? HSG_ZM_L64_DJ : HSG_ZM_DJ;   // J/H planes in flight
   static constexpr int NC1 = DS + 2;              // ring C1: planes k, k+1 live + DS in flight
@@ -244,7 +245,10 @@ struct Th {
   int grow_halo;              // HALO edge threads: element offset of the halo row they fetch (row gy-1 or gy+1, periodic)
   int edge;                   // HALO: -1 = lowest row of the strip, +1 = highest row, 0 = interior
   uint32_t row, rowp, rowm;   // byte offsets inside a shared [y][j] array: own row, row y+1, row y-1 at j0
-  uint32_t row0;              // own row at j0 inside an array without halo rows (ring C0)
+  uint32_t row0;              // own row at j0 inside an array without halo rows (ring C0, J/H arrays)
+  uint32_t jedge0;            // J/H arrays: own row at j0-1 (periodic)
+  uint32_t jym0, jym1;        // J/H arrays: offset of row y-1 at j0 relative to the OTHER colour's Jy array, for the colour-0 /
+                              // colour-1 update (strips: the lowest row reads the halo rows at the end of the ring slot)
   uint32_t edge0, edge1;      // own row at j0-1 and j0+V (periodic): the x neighbour outside the thread's V sites
   uint32_t halo;              // HALO edge threads: byte offset of the halo row they fill (== rowm or rowp)
   uint32_t push;              // HALO edge threads: cluster address of X0[0], component 0, halo row at j0 in the neighbour CTA
@@ -264,6 +268,7 @@ struct JAddr {
   uint32_t own_h;    // own colour, this plane: Hx, Hy, Hz at +0, +CJB, +2CJB
   uint32_t oth_xy;   // other colour, this plane: Jx, Jy              (bonds from -x, -y)
   uint32_t oth_z;    // other colour, plane below: Jz                 (bond from -z)
+  uint32_t ym;       // offset of row y-1 at j0 from the other colour's Jy array (th.jym0 / th.jym1)
 };
 
 // Local field of V sites of one colour in plane zp, accumulated in the order H, x+, x-, y+, y-, z+, z-
@@ -280,25 +285,25 @@ __device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&o
                                              const JAddr& ja, const Th& th, int off, const HbPar& hp, uint32_t site0, EAcc& ea) {
   const uint32_t edge = off ? th.edge1 : th.edge0;
   float Jxp[V], Jxm[V], Jyp[V], Jym[V], Jzp[V], Jzm[V];
-  lds<V>(Jxp, ja.own_xy + th.row);
-  lds<V>(Jyp, ja.own_xy + CJB + th.row);
-  lds<V>(Jzp, ja.own_z + th.row);
+  lds<V>(Jxp, ja.own_xy + th.row0);
+  lds<V>(Jyp, ja.own_xy + CJB + th.row0);
+  lds<V>(Jzp, ja.own_z + th.row0);
   {
     float t[V];
-    lds<V>(t, ja.oth_xy + th.row);
-    const float te = lds1(ja.oth_xy + th.edge0);
+    lds<V>(t, ja.oth_xy + th.row0);
+    const float te = lds1(ja.oth_xy + th.jedge0);
 #pragma unroll
     for (int e = 0; e < V; ++e) Jxm[e] = off ? t[e] : (e > 0 ? t[e > 0 ? e - 1 : 0] : te);
   }
-  lds<V>(Jym, ja.oth_xy + CJB + th.rowm);
-  lds<V>(Jzm, ja.oth_z + th.row);
+  lds<V>(Jym, ja.oth_xy + CJB + ja.ym);
+  lds<V>(Jzm, ja.oth_z + th.row0);
   float h[3][V];
   float Hs[3][V];
   const uint32_t xs_p = xs + th.rowp, xs_m = xs + th.rowm, xs_e = xs + edge;
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
     float Hm[V], yp[V], ym[V];
-    lds<V>(Hm, ja.own_h + mu * CJB + th.row);
+    lds<V>(Hm, ja.own_h + mu * CJB + th.row0);
     lds<V>(yp, xs_p + mu * CSB);
     lds<V>(ym, xs_m + mu * CSB);
     const float se = lds1(xs_e + mu * CSB);
@@ -382,19 +387,22 @@ __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __res
                        ::"r"(dB), "l"(src + 11 * C::CSG), "r"(JBB), "r"(bar), "l"(pol) : "memory");
         }
       } else {
+        // strip-major J/H layout (hsg_layout.cuh): the twelve arrays of this strip of the plane are contiguous; the row
+        // y0-1 of the two Jy arrays comes from the last row of the strip below.  Four copies, one per lane.
         constexpr uint32_t ROWB = 4u * C::Lh, STRIPB = 4u * C::YSv * C::Lh;
         const int lane = (int)threadIdx.x;
         if (lane == 0)
           asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(12u * STRIPB + 2u * ROWB) : "memory");
         __syncwarp();
-        if (lane < 14) {
-          const int arr = lane < 12 ? lane : (lane == 12 ? 1 : 6);           // halo rows: colour-0 Jy, colour-1 Jy
-          const uint32_t dbase = arr < 11 ? dA + (uint32_t)arr * JBB : dB;
-          const uint32_t dst = lane < 12 ? dbase + ROWB : dbase;
-          const int srow = lane < 12 ? sm.y0 : (sm.y0 + L - 1) % L;
-          const uint32_t bytes = lane < 12 ? STRIPB : ROWB;
+        if (lane < 4) {
+          const int strip = sm.y0 / C::YSv, below = (strip + C::NCL - 1) % C::NCL;
+          const float* blk = src + (size_t)strip * 12 * C::CSJ;
+          const float* blo = src + (size_t)below * 12 * C::CSJ + (size_t)(C::YSv - 1) * C::Lh;
+          const uint32_t dst = lane == 0 ? dA : lane == 1 ? dB : dA + 11u * JBB + (uint32_t)(lane - 2) * ROWB;
+          const float* from = lane == 0 ? blk : lane == 1 ? blk + 11 * C::CSJ : blo + (lane == 2 ? 1 : 6) * C::CSJ;
+          const uint32_t bytes = lane == 0 ? 11u * STRIPB : lane == 1 ? STRIPB : ROWB;
           asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                       ::"r"(dst), "l"(src + (size_t)arr * C::CSG + (size_t)srow * C::Lh), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+                       ::"r"(dst), "l"(from), "r"(bytes), "r"(bar), "l"(pol) : "memory");
         }
       }
     }
@@ -528,7 +536,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     const uint32_t par = (uint32_t)(k & 1);
     {
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * k));
-      const JAddr ja = {ak, bk, ak + 2 * CJB, ak + 5 * CJB, ak1 + 7 * CJB};
+      const JAddr ja = {ak, bk, ak + 2 * CJB, ak + 5 * CJB, ak1 + 7 * CJB, th.jym0};
       update_sites<CSB, CJB, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % C::NC1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + k * PS + mu * CS, R[mu]);
@@ -538,7 +546,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     if (k >= 1) wait_halo(par ^ 1u);                   // (step 0's rows are pushed again in the tail: consumed unread)
     if (k >= 2) {     // colour 1 of plane k-1
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * (k - 1)));
-      const JAddr ja = {ak1 + 5 * CJB, ak1 + 7 * CJB, ak1 + 8 * CJB, ak1, bk2};
+      const JAddr ja = {ak1 + 5 * CJB, ak1 + 7 * CJB, ak1 + 8 * CJB, ak1, bk2, th.jym1};
       float N1[3][V];
       update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
@@ -575,7 +583,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     const uint32_t b2 = sm.jb + ((uint32_t)(nd + C::NJB - 1) % C::NJB) * JBB;        // colour-0 Jz of plane k-2
     const int z1 = kk == 0 ? L - 1 : 0;
     const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * z1));
-    const JAddr ja = {a1 + 5 * CJB, a1 + 7 * CJB, a1 + 8 * CJB, a1, b2};
+    const JAddr ja = {a1 + 5 * CJB, a1 + 7 * CJB, a1 + 8 * CJB, a1, b2, th.jym1};
     float N1[3][V];
     update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
@@ -639,6 +647,13 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
     th.rowp = 4u * (uint32_t)(((ly + 1 == L) ? 0 : ly + 1) * C::Lh + th.j0);
     th.rowm = 4u * (uint32_t)(((ly == 0) ? L - 1 : ly - 1) * C::Lh + th.j0);
     th.edge = 0; th.grow_halo = 0; th.halo = 0; th.push = 0; th.push_bar = 0;
+  }
+  th.jedge0 = 4u * (uint32_t)(ly * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1));
+  if (C::HALO && ly == 0) {       // row y0-1 of the other colour's Jy: halo rows behind the 11 arrays of the ring-A slot
+    th.jym0 = 4u * (uint32_t)((11 - 6) * C::CSJ + C::Lh + th.j0);    // colour-0 update reads colour-1 Jy (array 6), halo row 1
+    th.jym1 = 4u * (uint32_t)((11 - 1) * C::CSJ + th.j0);            // colour-1 update reads colour-0 Jy (array 1), halo row 0
+  } else {
+    th.jym0 = th.jym1 = 4u * (uint32_t)(((ly == 0) ? L - 1 : ly - 1) * C::Lh + th.j0);
   }
   th.edge0 = 4u * (uint32_t)((ly + HR) * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1));
   th.edge1 = 4u * (uint32_t)((ly + HR) * C::Lh + ((th.j0 + V == C::Lh) ? 0 : th.j0 + V));
