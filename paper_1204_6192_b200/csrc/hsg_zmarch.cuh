@@ -370,7 +370,11 @@ struct Stream {        // J/H plane stream: index q -> plane (q-1) mod L
 template <class C, int L, class SmemT>
 __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __restrict__ jh_d, Stream& st, int nd, uint64_t pol) {
   constexpr uint32_t JAB = 4u * C::JA, JBB = 4u * C::CSJ;
-  if (threadIdx.x < 32) {
+  // issuing a bulk copy costs its warp tens of cycles, and the CTA waits for its slowest warp at the step barrier: the
+  // copies of a plane are issued by the first lanes of different warps (two for a whole plane, four for a strip)
+  constexpr bool TWO = !C::HALO && C::NT > 32;
+  constexpr bool FOUR = C::HALO && C::NT >= 128;
+  if (FOUR ? ((threadIdx.x & 31u) == 0 && threadIdx.x < 128) : (threadIdx.x < 32 || (TWO && threadIdx.x == 32))) {
     const int upto = min(nd + C::DJ, st.total - 1);
     while (st.issued < upto) {
       ++st.issued;
@@ -383,17 +387,18 @@ __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __res
           asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(JAB + JBB) : "memory");
           asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
                        ::"r"(dA), "l"(src), "r"(JAB), "r"(bar), "l"(pol) : "memory");
+        }
+        if (threadIdx.x == (TWO ? 32 : 0))     // (its complete_tx may land before the expect_tx: the phase still needs that arrive)
           asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
                        ::"r"(dB), "l"(src + 11 * C::CSG), "r"(JBB), "r"(bar), "l"(pol) : "memory");
-        }
       } else {
         // strip-major J/H layout (hsg_layout.cuh): the twelve arrays of this strip of the plane are contiguous; the row
         // y0-1 of the two Jy arrays comes from the last row of the strip below.  Four copies, one per lane.
         constexpr uint32_t ROWB = 4u * C::Lh, STRIPB = 4u * C::YSv * C::Lh;
-        const int lane = (int)threadIdx.x;
-        if (lane == 0)
+        const int lane = FOUR ? (int)(threadIdx.x >> 5) : (int)threadIdx.x;      // which of the four copies
+        if (lane == 0)       // (a complete_tx that lands before this expect_tx is fine: the phase still needs the arrive)
           asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(12u * STRIPB + 2u * ROWB) : "memory");
-        __syncwarp();
+        if (!FOUR) __syncwarp();
         if (lane < 4) {
           const int strip = sm.y0 / C::YSv, below = (strip + C::NCL - 1) % C::NCL;
           const float* blk = src + (size_t)strip * 12 * C::CSJ;
