@@ -10,7 +10,8 @@ hsg_sweep(n_or, n_hb) + hsg_pt_swap (energies + swaps) + hsg_measure (E, m, q(0)
 `e2e`   = the same metric over one "execution round" driven through the C ABI from HOST
           buffers: J, H and the start spins are copied from pinned host memory, K steps run with the
           observables of every step read back to the host, and the final spins are read back — all inside
-          the timed region; bytes per step = round bytes / K.
+          the timed region; bytes per step = round bytes / K.  The round runs as shards of disorder samples,
+          one context and stream each, so that the copies of one shard overlap the sweeps of the others.
 `roofline` is for the sweep kernel (the dominant one): algorithmic bytes / CUDA-event time.
 `cpu_baseline` = the oracle (oracle/, as it stands) timed on the host cores on a bounded sample.
 Rank r of an N-GPU run owns its own D samples (sample_offset = r*D): weak scaling, no data-path collective.
@@ -245,22 +246,42 @@ def main_ours(args, cfg, temps):
         S_h = torch.empty(S0.shape, dtype=torch.float32).pin_memory(); S_h.copy_(S0); del S0
         out_h = [torch.empty(o.shape, dtype=o.dtype).pin_memory() for o in outs] + [torch.empty(acc.shape, dtype=i32).pin_memory()]
         S_back = torch.empty(S_h.shape, dtype=torch.float32).pin_memory()
-        S_dev = eng._new(S_h.shape, torch.float32)
-        J_dev = eng._new(J_h.shape, torch.float32); H_dev = eng._new(J_h.shape, torch.float32) if H_h is not None else None
+        # The round runs as K shards of D/K disorder samples, one hsg context and one CUDA stream each (samples are
+        # independent: DESIGN.md §8; sample_offset keeps every random stream that of the global sample), so the H2D
+        # and D2H copies of one shard overlap the sweeps of the others.
+        K = args.e2e_shards if args.e2e_shards > 0 else (8 if D % 8 == 0 and D >= 16 else 4 if D % 4 == 0 and D >= 8 else 1)
+        assert D % K == 0, "--e2e-shards must divide the number of samples"
+        Ds = D // K
+        shards = []
+        for k in range(K):
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                e = hsg.hsg_create(L, Ds, O, temps, cfg["seed"], sample_offset=off + k * Ds, stream=st, kernel=args.kernel)
+                if args.no_fuse_energy:
+                    e.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
+                sl = slice(k * Ds, (k + 1) * Ds)
+                dev = dict(J=e._new(J_h[sl].shape, torch.float32), H=(e._new(J_h[sl].shape, torch.float32) if H_h is not None else None),
+                           S=e._new(S_h[sl].shape, torch.float32),
+                           outs=(e._new((Ds, O, T), f64), e._new((Ds, O, T, 3), f64), e._new((Ds, e.P, T, 3, 3), f64), e._new((Ds, e.P, T, 3, 3, 2), f64)),
+                           acc=e._new((Ds, O, max(T - 1, 0)), i32))
+            shards.append((e, st, sl, dev))
+
         def round_():
-            J_dev.copy_(J_h, non_blocking=True)
-            if H_dev is not None:
-                H_dev.copy_(H_h, non_blocking=True)
-            S_dev.copy_(S_h, non_blocking=True)
-            eng.set_disorder(J_dev, H_dev); eng.set_spins(S_dev)
-            for _ in range(args.steps):
-                eng.sweep(n_or, n_hb)
-                eng.pt_swap(out=acc)
-                eng.measure(out=outs)
-                for h, d in zip(out_h, list(outs) + [acc]):
-                    h.copy_(d, non_blocking=True)
-            eng.get_spins(out=S_dev)
-            S_back.copy_(S_dev, non_blocking=True)
+            for e, st, sl, dev in shards:
+                with torch.cuda.stream(st):
+                    dev["J"].copy_(J_h[sl], non_blocking=True)
+                    if dev["H"] is not None:
+                        dev["H"].copy_(H_h[sl], non_blocking=True)
+                    dev["S"].copy_(S_h[sl], non_blocking=True)
+                    e.set_disorder(dev["J"], dev["H"]); e.set_spins(dev["S"])
+                    for _ in range(args.steps):
+                        e.sweep(n_or, n_hb)
+                        e.pt_swap(out=dev["acc"])
+                        e.measure(out=dev["outs"])
+                        for h, d in zip(out_h, list(dev["outs"]) + [dev["acc"]]):
+                            h[sl].copy_(d, non_blocking=True)
+                    e.get_spins(out=dev["S"])
+                    S_back[sl].copy_(dev["S"], non_blocking=True)
         round_()                                            # warm-up round
         barrier()
         t0 = time.perf_counter()
@@ -275,7 +296,8 @@ def main_ours(args, cfg, temps):
         d2h = S_back.numel() * 4 + args.steps * sum(h.numel() * h.element_size() for h in out_h)
         e2e = {"value": e2e_s * 1e9 / ((n_or + n_hb) * R * N * args.steps), "unit": UNIT,
                "h2d_bytes_per_step": h2d // args.steps, "d2h_bytes_per_step": d2h // args.steps,
-               "what": f"one round of {args.steps} steps: J,H,spins H2D from pinned host + steps with per-step observables D2H + spins D2H"}
+               "what": f"one round of {args.steps} steps: J,H,spins H2D from pinned host + steps with per-step observables D2H + spins D2H; "
+                       f"{K} sample shard(s), one context and stream each"}
 
     if rank != 0:
         if dist is not None:
@@ -343,6 +365,7 @@ def main():
     ap.add_argument("--n-or", type=int, default=None, help="override the over-relaxation sweeps per step (OR-only / HB-only timing points)")
     ap.add_argument("--n-hb", type=int, default=None, help="override the heat-bath sweeps per step")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-shards", type=int, default=0, help="sample shards (contexts + streams) of the end-to-end round; 0 = 8 or 4 if they divide the samples")
     ap.add_argument("--no-measure", action="store_true")
     ap.add_argument("--no-fuse-energy", action="store_true", help="separate energy reduction kernel instead of the fused final sweep")
     ap.add_argument("--cpu-steps", type=int, default=3, help="oracle steps timed for cpu_baseline")
