@@ -111,12 +111,14 @@ int hsg_get_spins(hsg_ctx* ctx, float* S_dev);
  * The heat-bath sweep counter advances by one per HB sweep. */
 int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb);
 
-/* Total energy (Eq. 1) of every system, fp64, E_dev [D][O][T] by temperature index. */
+/* Total energy (Eq. 1, every nearest-neighbour bond once) of every system, E_dev [D][O][T] by temperature
+ * index.  Precision as PAPER.md:185: the site terms s_i.h_i (odd sites, h_i the local field of PAPER.md:37) and s_i.H_i
+ * (even sites) in single precision, their sum over the lattice in double. */
 int hsg_energy(hsg_ctx* ctx, double* E_dev);
 
 /* One parallel-tempering pass (Eq. 4): for each (sample, replica), pairs (t, t+1) for
  * t = 0..T-2 in this order, swap accepted with probability min[1, exp(dbeta*dE)],
- * dE = E_{t+1}-E_t, dbeta = beta_{t+1}-beta_t, energies recomputed from the spins in fp64.
+ * dE = E_{t+1}-E_t, dbeta = beta_{t+1}-beta_t in fp64, energies as hsg_energy recomputed from the spins.
  * accepted_dev [D][O][T-1] int32 (1 = swapped) or NULL.  The PT counter advances by one per call. */
 int hsg_pt_swap(hsg_ctx* ctx, int32_t* accepted_dev);
 

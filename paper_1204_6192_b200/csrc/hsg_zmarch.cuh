@@ -1,6 +1,7 @@
 // hsg_zmarch.cuh — the fused z-marching sweep kernel.
 //
-// One launch runs a whole hsg_sweep(n_or, n_hb) call.  A CTA owns G configuration slots of ONE disorder
+// One launch runs a whole hsg_sweep(n_or, n_hb) call (at L = 32 and 16 the heat-bath sweeps are a second launch with
+// fewer sites per thread, see zmarch_launch).  A CTA owns G configuration slots of ONE disorder
 // sample and marches them together through the lattice planes z = 0..L-1, updating colour 0 of plane k
 // and then colour 1 of plane k-1 in step k, so that every spin is read once and written once per sweep
 // and the result is exactly the global two-colour sweep of PAPER.md:141-146 (colour 1 of a plane is
@@ -14,21 +15,24 @@
 //   * Spin planes are streamed global -> shared memory by per-thread cp.async copies of the thread's OWN
 //     column, DS steps ahead of their use (rings C1 = old colour-1 planes, C0 = old colour-0 planes).
 //     Completion is tracked per thread by cp.async groups, which (unlike register loads, whose scoreboard is
-//     shared with younger loads) lets a step wait for the oldest stage while DS-1 younger ones stay in
-//     flight: the bytes in flight per SM, not the issue rate, bound this kernel (Little's law).
+//     shared with younger loads) lets a step wait for the oldest stage while DS-1 younger ones stay in flight.
 //   * In-plane neighbours (rows y-1, y+1 and the one x neighbour outside the thread's V sites) are read
 //     from shared memory: ring C1 holds the old colour-1 spins of plane k, X0 (double-buffered) the new
-//     colour-0 spins of plane k-1; one __syncthreads per step.
+//     colour-0 spins of plane k-1; one barrier per step.
 //   * Couplings and fields of the sample stream through shared-memory rings filled by bulk async copies
-//     (cp.async.bulk, mbarrier completion) issued DJ steps ahead by thread 0, and are shared by the G
-//     systems of the CTA (PAPER.md:161's R_TO idea).  Eleven of the twelve arrays of a plane live for two
-//     steps (ring A); the +z couplings of colour 0 live for three (ring B).
+//     (cp.async.bulk, mbarrier completion) issued DJ steps ahead, and are shared by the G systems of the CTA
+//     (PAPER.md:161's R_TO idea).  Eleven of the twelve arrays of a plane live for two steps (ring A); the +z
+//     couplings of colour 0 live for three (ring B).  Issuing a bulk copy costs its warp tens of cycles and the
+//     whole CTA waits for its slowest warp at the step barrier, so the copies of a plane are issued by lane 0 of
+//     different warps (two for a whole plane, four for a strip).
 //   * Lattices whose planes do not fit one SM's shared memory (L = 64) are split into L/YS strips of YS rows;
-//     the strips of a system group are the CTAs of one thread-block cluster.  Every shared array then carries
-//     halo rows: the old colour-1 halo rows are fetched from global memory by the edge threads (the owner
+//     the strips of a system group are the CTAs of one thread-block cluster.  Every shared spin array then
+//     carries halo rows: the old colour-1 halo rows are fetched from global memory by the edge threads (the owner
 //     overwrites them only two cluster barriers later), the new colour-0 halo rows are pushed into the
-//     neighbour CTA's shared memory (st.shared::cluster) by the thread that computed them, and the
-//     one-per-step __syncthreads becomes a cluster barrier (arrive.release / wait.acquire).
+//     neighbour CTA's shared memory (st.async, counted on an mbarrier of that CTA) by the thread that computed
+//     them, and the step barrier becomes a __syncthreads plus a split, relaxed cluster barrier (step_end / step_wait).
+//     The J/H layout is strip-major (hsg_layout.cuh): two bulk copies per strip and plane, plus the two Jy rows below the strip.
+//   * In the final sweep of a call the kernel also reduces E and m of every system.
 #pragma once
 #include <cuda_runtime.h>
 #include "hsg_layout.cuh"
