@@ -48,12 +48,15 @@ def _peaks():
 
 
 def _traffic(workload, kernel):
-    """dram bytes per sweep-kernel launch from the committed ncu capture (profiles/traffic.json), or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes per sweep-kernel launch from the committed ncu capture (profiles/traffic.csv), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
-        return json.load(open(p)).get(f"{workload}:{kernel}")
+        for line in open(p):
+            if line.startswith(f"{workload}:{kernel},"):
+                return float(line.strip().split(",")[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
