@@ -76,11 +76,14 @@ CONFIGS = {
 }
 
 
-def make_config(name: str, n_samples: int | None = None, sample_offset: int = 0):
-    """Return (cfg, temps, J, H) for a BASELINE.json config; H is None for zero field."""
+def make_config(name: str, n_samples: int | None = None, sample_offset: int = 0, h_r: float | None = None):
+    """Return (cfg, temps, J, H) for a BASELINE.json config; H is None for zero field.  ``h_r`` overrides the field
+    strength (c3's scan {0.05, 0.1, 0.2}: the same couplings and the same unit-variance field draws, scaled)."""
     cfg = dict(CONFIGS[name])
     if n_samples is not None:
         cfg["n_samples"] = n_samples
+    if h_r is not None:
+        cfg["h_r"] = h_r
     if cfg["t_min"] == cfg["t_max"]:      # Table-1 workload: all systems at one temperature; ladder must ascend
         temps = (cfg["t_min"] * (1.0 + 1e-6 * np.arange(cfg["n_temps"]))).astype(np.float32)
     else:

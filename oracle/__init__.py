@@ -77,9 +77,15 @@ def lib() -> C.CDLL:
         L.orc_get_spins.argtypes = [vp, vp]
         L.orc_sweep.argtypes = [vp, C.c_int, C.c_int, C.c_int]
         L.orc_energy.argtypes = [vp, vp]
+        L.orc_energy_plain.argtypes = [vp, vp]
         L.orc_pt_swap.argtypes = [vp, vp]
         L.orc_measure.argtypes = [vp, vp, vp, vp, vp]
         L.orc_get_state.argtypes = [vp, vp, vp]
+        L.orc_chi_field.argtypes = [vp, vp, C.c_int, C.c_int]; L.orc_chi_field.restype = C.c_int
+        L.orc_measure_chiral.argtypes = [vp, vp, vp, vp]
+        L.orc_xi_second_moment.argtypes = [f64, f64, C.c_int]; L.orc_xi_second_moment.restype = f64
+        L.orc_pt_diag_reset.argtypes = [vp]
+        L.orc_pt_diag_get.argtypes = [vp, vp, vp, vp, vp]
         L.orc_set_counters.argtypes = [vp, vp]
         _LIB = L
     return _LIB
@@ -127,6 +133,11 @@ def hb_draw(h, beta, u1, u2, precision=64) -> np.ndarray:
     h = np.ascontiguousarray(h, dtype=dt); out = np.empty(3, dtype=dt)
     getattr(lib(), f"orc_hb_draw_f{precision}")(_p(h), float(beta), float(u1), float(u2), _p(out))
     return out
+
+
+def xi_second_moment(chi_0: float, chi_k: float, L: int) -> float:
+    """Eq. (8) / Eq. (15): xi = sqrt(chi(0)/chi(k_min) - 1) / (2 sin(k_min/2)), |k_min| = 2 pi/L."""
+    return lib().orc_xi_second_moment(float(chi_0), float(chi_k), int(L))
 
 
 def hb_sample(h, beta, seed, n, precision=64) -> np.ndarray:
@@ -182,6 +193,12 @@ class Oracle:
         lib().orc_energy(self._h, _p(E))
         return E
 
+    def energy_plain(self) -> np.ndarray:
+        """Eq. (1) as written: forward bonds once, every product and the sum in fp64 (the plain definition)."""
+        E = np.empty((self.D, self.O, self.T), dtype=np.float64)
+        lib().orc_energy_plain(self._h, _p(E))
+        return E
+
     def pt_swap(self) -> np.ndarray:
         acc = np.empty((self.D, self.O, max(self.T - 1, 0)), dtype=np.int32)
         lib().orc_pt_swap(self._h, _p(acc))
@@ -195,6 +212,36 @@ class Oracle:
         qk = np.empty((self.D, P, self.T, 3, 3, 2), dtype=np.float64)
         lib().orc_measure(self._h, _p(E), _p(M), _p(q0), _p(qk))
         return E, M, q0, qk
+
+    def chi_field(self, plain=False) -> np.ndarray:
+        """Summands of Eq. (10) from replicas 0..3: chi[D][T][2 (k=0, k_min)][3 (chi_1, chi_2, chi_3)][2 (re, im)].
+        plain=True: the O(N^2) double sum as printed; False: the factored form (identical numbers, pinned)."""
+        chi = np.empty((self.D, self.T, 2, 3, 2), dtype=np.float64)
+        if lib().orc_chi_field(self._h, _p(chi), int(bool(plain)), int(self.n_threads)) != 0:
+            raise ValueError("chi_field needs at least four replicas")
+        return chi
+
+    def measure_chiral(self, want_kappa=False):
+        """Chiral overlaps of Eqs. (12), (13): qc0[D][P][T][3], qck[D][P][T][3][2]; optionally kappa[D][O][T][3][L][L][L]."""
+        P = self.O * (self.O - 1) // 2
+        qc0 = np.empty((self.D, P, self.T, 3), dtype=np.float64)
+        qck = np.empty((self.D, P, self.T, 3, 2), dtype=np.float64)
+        kap = np.empty((self.D, self.O, self.T, 3, self.L, self.L, self.L), dtype=np.float64) if want_kappa else None
+        lib().orc_measure_chiral(self._h, _p(qc0), _p(qck), _p(kap))
+        return (qc0, qck, kap) if want_kappa else (qc0, qck)
+
+    def pt_diag_reset(self):
+        """Start (or restart) the parallel-tempering diagnostics of PAPER.md:197 / Fig. 3; every later pt_swap() is counted."""
+        lib().orc_pt_diag_reset(self._h)
+
+    def pt_diag_get(self):
+        """(moved[D][O][T] by temperature index, traversals[D][O][T] by configuration slot, n_pass, p_diff[T])."""
+        moved = np.empty((self.D, self.O, self.T), dtype=np.int64)
+        trav = np.empty((self.D, self.O, self.T), dtype=np.int64)
+        n = C.c_uint64(0)
+        p = np.empty(self.T, dtype=np.float64)
+        lib().orc_pt_diag_get(self._h, _p(moved), _p(trav), C.addressof(n), _p(p))
+        return moved, trav, int(n.value), p
 
     def get_state(self):
         perm = np.empty((self.D, self.O, self.T), dtype=np.int32)

@@ -256,6 +256,12 @@ struct Sim {
   std::vector<Real> S;                 // [D][O][slot][3][N]
   std::vector<int32_t> conf_of_temp;   // [D][O][T]
   bool have_disorder = false, have_spins = false;
+  // parallel-tempering diagnostics of PAPER.md:197 / Fig. 3, see pt_diag_reset()
+  bool diag_on = false;
+  uint64_t diag_passes = 0;
+  std::vector<int64_t> diag_moved;     // [D][O][T] by TEMPERATURE index: passes after which the copy that held T_t had left it
+  std::vector<int64_t> diag_trav;      // [D][O][slot] end-to-end traversals T_1 <-> T_{R_T} of every configuration
+  std::vector<int8_t> diag_last;       // [D][O][slot] end point touched last: +1 = T_1, -1 = T_{R_T}, 0 = none yet
 
   Sim(int L_, int D_, int O_, int T_, const float* temps_, uint64_t seed_, uint64_t off)
       : L(L_), D(D_), O(O_), T(T_), N((long)L_ * L_ * L_), seed(seed_), sample_offset(off),
@@ -384,11 +390,37 @@ struct Sim {
       E[((size_t)d * O + o) * T + t] = energy_of(spins_of_temp(d, o, t), d);
   }
 
+  // PAPER.md:26 Eq. (1) exactly as written, the plain definition:  E = - sum_<ij> J_ij s_i.s_j - sum_i H_i.s_i ,
+  // every nearest-neighbour bond once (the three forward bonds x+, y+, z+ of every site; reading 1), every product
+  // and the whole sum in double from the stored spins, sites in index order.  No local field, no colours, no
+  // single-precision intermediate: this is what energy_of() (the PAPER.md:185 reading the moves and the
+  // parallel-tempering decisions use) is pinned against, and what the GPU energies are bounded against.
+  double energy_plain_of(const Real* s, int d) const {
+    const float* Jd = &J[(size_t)d * 3 * N];
+    const float* Hd = &H[(size_t)d * 3 * N];
+    double E = 0.0;
+    for (long i = 0; i < N; ++i) {
+      for (int dir = 0; dir < 3; ++dir) {
+        const long ip = nbr(i, dir, +1);
+        double dot = 0.0;
+        for (int c = 0; c < 3; ++c) dot += (double)s[(size_t)c * N + i] * (double)s[(size_t)c * N + ip];
+        E -= (double)Jd[(size_t)dir * N + i] * dot;
+      }
+      for (int c = 0; c < 3; ++c) E -= (double)Hd[(size_t)c * N + i] * (double)s[(size_t)c * N + i];
+    }
+    return E;
+  }
+  void energy_plain(double* E /*[D][O][T]*/) {
+    for (int d = 0; d < D; ++d) for (int o = 0; o < O; ++o) for (int t = 0; t < T; ++t)
+      E[((size_t)d * O + o) * T + t] = energy_plain_of(spins_of_temp(d, o, t), d);
+  }
+
   // Parallel tempering, Eq. (4): pairs (t, t+1) from the lowest temperature upwards,
   // accept with min[1, exp(dbeta*dE)], dE = E_{t+1}-E_t, dbeta = beta_{t+1}-beta_t.  One chain per (d,o).
   void pt_swap(int32_t* accepted /*[D][O][T-1] or null*/) {
     std::vector<double> E((size_t)D * O * T);
     energy(E.data());
+    const std::vector<int32_t> before = conf_of_temp;          // (diagnostics only)
     uint32_t k[2]; key(k);
     for (int d = 0; d < D; ++d) for (int o = 0; o < O; ++o) {
       double* Eg = &E[((size_t)d * O + o) * T];
@@ -405,6 +437,44 @@ struct Sim {
       }
     }
     ++k_pt;
+    if (diag_on) pt_diag_update(before);
+  }
+
+  // ---- Parallel-tempering diagnostics (Fig. 3) ----
+  // p_diff(T_t): "the probability that, after a parallel tempering update, a copy of the system at T_t will diffuse to
+  // neighboring temperatures": per pass and (d,o), the copy (configuration slot) that held T_t before the pass holds
+  // another temperature after it.  Tunnelling: "a replica travels a closed loop between the temperature end points T_1
+  // and T_{R_T}": every arrival of a configuration at one end point after it last touched the OTHER one is one
+  // traversal; a closed loop = two traversals (N_tunn = traversals / 2, integer division, per configuration).
+  void pt_diag_touch() {
+    for (int g = 0; g < D * O; ++g)
+      for (int e = 0; e < 2; ++e) {
+        const int t_end = e == 0 ? 0 : T - 1;
+        const int8_t tag = e == 0 ? 1 : -1;
+        const size_t s = (size_t)g * T + conf_of_temp[(size_t)g * T + t_end];
+        if (diag_last[s] == -tag) ++diag_trav[s];
+        diag_last[s] = tag;
+      }
+  }
+  void pt_diag_reset() {
+    diag_on = true; diag_passes = 0;
+    diag_moved.assign((size_t)D * O * T, 0); diag_trav.assign((size_t)D * O * T, 0); diag_last.assign((size_t)D * O * T, 0);
+    pt_diag_touch();                      // the configurations that START at an end point have touched it
+  }
+  void pt_diag_update(const std::vector<int32_t>& before) {
+    for (size_t r = 0; r < before.size(); ++r) diag_moved[r] += (conf_of_temp[r] != before[r]) ? 1 : 0;
+    ++diag_passes;
+    pt_diag_touch();
+  }
+  void pt_diag_get(int64_t* moved, int64_t* trav, uint64_t* n_pass, double* p_diff /*[T]*/) const {
+    if (moved) std::copy(diag_moved.begin(), diag_moved.end(), moved);
+    if (trav) std::copy(diag_trav.begin(), diag_trav.end(), trav);
+    if (n_pass) *n_pass = diag_passes;
+    if (p_diff) for (int t = 0; t < T; ++t) {
+      double acc = 0.0;
+      for (int g = 0; g < D * O; ++g) acc += (double)diag_moved[(size_t)g * T + t];
+      p_diff[t] = diag_passes ? acc / ((double)D * O * (double)diag_passes) : 0.0;
+    }
   }
 
   // Measurements: E per system; m = (1/N) sum_i s_i; overlap tensor PAPER.md:53-58 Eqs. (5),(6)
@@ -443,6 +513,149 @@ struct Sim {
     }
   }
 };
+
+// --------------------------------------------------------------------------------------
+// Field-case observables, Eqs. (9)-(11): four real replicas (1),(2),(3),(4) = replicas 0,1,2,3 of a
+// sample, all at the same temperature index.  One measurement contributes the summands of Eq. (10):
+//   chi_1(k) = sum_{i,j} sum_{mu,nu} s_i^{mu(1)} s_j^{nu(1)} s_i^{mu(2)} s_j^{nu(2)} e^{ik.(R_i-R_j)}
+//   chi_2(k) = sum_{i,j} sum_{mu,nu} s_i^{mu(1)} s_j^{nu(1)} s_i^{mu(3)} s_j^{nu(4)} e^{ik.(R_i-R_j)}
+//   chi_3(k) = sum_{i,j} sum_{mu,nu} s_i^{mu(1)} s_j^{nu(2)} s_i^{mu(3)} s_j^{nu(4)} e^{ik.(R_i-R_j)}
+// for k = 0 and k_min = (2 pi/L)(1,0,0); the thermal average <.> is the caller's running mean over
+// measurements and Eq. (11) chi_SG(k) = (1/N)[chi_1 - 2 chi_2 + chi_3]_J its linear combination.  All arithmetic in
+// double.  Output chi[D][T][2 (k = 0, k_min)][3 (chi_1, chi_2, chi_3)][2 (re, im)].
+//
+// chi_field_plain: the definition written out — the double sum over sites and components, nothing factored.  O(N^2).
+// chi_field      : the same numbers from A_ab(k) = sum_i (s_i^(a) . s_i^(b)) e^{ik x_i}; in Eq. (10) site i always
+//                  carries the index mu in both of its factors and site j the index nu, so the sums over (i, mu) and
+//                  (j, nu) factor:  chi_1 = |A_12|^2, chi_2 = A_13 conj(A_14), chi_3 = A_13 conj(A_24).  O(N); pinned
+//                  against chi_field_plain in tests/test_oracle_field_chiral.py.
+// --------------------------------------------------------------------------------------
+template <class Real>
+void chi_field_plain_one(Sim<Real>& sim, int d, int t, double* out /*[2][3][2]*/) {
+  const long N = sim.N; const int L = sim.L;
+  const Real* s[4];
+  for (int r = 0; r < 4; ++r) s[r] = sim.spins_of_temp(d, r, t);
+  const double two_pi = 6.283185307179586476925286766559;
+  for (int ik = 0; ik < 2; ++ik) {
+    const double kx = ik == 0 ? 0.0 : two_pi / (double)L;
+    double acc[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+    for (long i = 0; i < N; ++i) for (long j = 0; j < N; ++j) {
+      const double ph = kx * (double)((i % L) - (j % L));
+      const double co = std::cos(ph), si = std::sin(ph);
+      for (int mu = 0; mu < 3; ++mu) for (int nu = 0; nu < 3; ++nu) {
+        const double i1 = (double)s[0][(size_t)mu * N + i], i2 = (double)s[1][(size_t)mu * N + i], i3 = (double)s[2][(size_t)mu * N + i];
+        const double j1 = (double)s[0][(size_t)nu * N + j], j2 = (double)s[1][(size_t)nu * N + j], j4 = (double)s[3][(size_t)nu * N + j];
+        const double c1 = i1 * j1 * i2 * j2;        // s_i^{mu(1)} s_j^{nu(1)} s_i^{mu(2)} s_j^{nu(2)}
+        const double c2 = i1 * j1 * i3 * j4;        // s_i^{mu(1)} s_j^{nu(1)} s_i^{mu(3)} s_j^{nu(4)}
+        const double c3 = i1 * j2 * i3 * j4;        // s_i^{mu(1)} s_j^{nu(2)} s_i^{mu(3)} s_j^{nu(4)}
+        acc[0][0] += c1 * co; acc[0][1] += c1 * si;
+        acc[1][0] += c2 * co; acc[1][1] += c2 * si;
+        acc[2][0] += c3 * co; acc[2][1] += c3 * si;
+      }
+    }
+    for (int c = 0; c < 3; ++c) { out[(ik * 3 + c) * 2] = acc[c][0]; out[(ik * 3 + c) * 2 + 1] = acc[c][1]; }
+  }
+}
+
+template <class Real>
+void chi_field_one(Sim<Real>& sim, int d, int t, double* out /*[2][3][2]*/) {
+  const long N = sim.N; const int L = sim.L;
+  const Real* s[4];
+  for (int r = 0; r < 4; ++r) s[r] = sim.spins_of_temp(d, r, t);
+  const double two_pi = 6.283185307179586476925286766559;
+  const int pa[4] = {0, 0, 0, 1}, pb[4] = {1, 2, 3, 3};     // A_12, A_13, A_14, A_24
+  for (int ik = 0; ik < 2; ++ik) {
+    double A[4][2];
+    for (int p = 0; p < 4; ++p) {
+      double re = 0.0, im = 0.0;
+      for (long i = 0; i < N; ++i) {
+        double dot = 0.0;
+        for (int mu = 0; mu < 3; ++mu) dot += (double)s[pa[p]][(size_t)mu * N + i] * (double)s[pb[p]][(size_t)mu * N + i];
+        const double ph = ik == 0 ? 0.0 : two_pi * (double)(i % L) / (double)L;
+        re += dot * std::cos(ph); im += dot * std::sin(ph);
+      }
+      A[p][0] = re; A[p][1] = im;
+    }
+    double* o = out + ik * 6;
+    o[0] = A[0][0] * A[0][0] + A[0][1] * A[0][1]; o[1] = 0.0;                                   // |A_12|^2
+    o[2] = A[1][0] * A[2][0] + A[1][1] * A[2][1]; o[3] = A[1][1] * A[2][0] - A[1][0] * A[2][1];  // A_13 conj(A_14)
+    o[4] = A[1][0] * A[3][0] + A[1][1] * A[3][1]; o[5] = A[1][1] * A[3][0] - A[1][0] * A[3][1];  // A_13 conj(A_24)
+  }
+}
+
+template <class Real>
+void chi_field_all(Sim<Real>& sim, double* chi, bool plain, int n_threads) {
+  const int D = sim.D, T = sim.T;
+  auto work = [&](int r0, int r1) {
+    for (int r = r0; r < r1; ++r) {
+      if (plain) chi_field_plain_one(sim, r / T, r % T, chi + (size_t)r * 12);
+      else chi_field_one(sim, r / T, r % T, chi + (size_t)r * 12);
+    }
+  };
+  const int n = D * T, nt = std::max(1, std::min(n_threads, n));
+  if (nt == 1) { work(0, n); return; }
+  std::vector<std::thread> th;
+  for (int k = 0; k < nt; ++k) th.emplace_back(work, n * k / nt, n * (k + 1) / nt);
+  for (auto& x : th) x.join();
+}
+
+// --------------------------------------------------------------------------------------
+// Chiral sector, Eqs. (12), (13):
+//   kappa_i^alpha = s_{i+alpha} . (s_i x s_{i-alpha}),  alpha = x, y, z (periodic)                              (12)
+//   q_c^alpha(k)  = (1/N) sum_i kappa_i^{alpha(a)} kappa_i^{alpha(b)} e^{ik.R_i}                               (13)
+// for replica pairs a < b at the same temperature, k = 0 and k_min = (2 pi/L)(1,0,0) for every alpha (the paper defines
+// one k_min; reading 22).  The local chirality is a per-site quantity of the spins and is formed
+// in the spins' precision Real with this fixed operation order:
+//   c = s_i x s_{i-alpha}:  c_x = fma(b_y, m_z, -(b_z*m_y)), c_y = fma(b_z, m_x, -(b_x*m_z)), c_z = fma(b_x, m_y, -(b_y*m_x))
+//   kappa = fma(p_z, c_z, fma(p_y, c_y, p_x*c_x)),   p = s_{i+alpha}, b = s_i, m = s_{i-alpha};
+// the product kappa^(a) kappa^(b) and the sums are double.  chi_CG (Eq. 14) and xi_c (Eq. 15) are the caller's averages.
+// Output qc0[D][P][T][3], qck[D][P][T][3][2 (re, im)].
+// --------------------------------------------------------------------------------------
+template <class Real>
+Real chirality(const Sim<Real>& sim, const Real* s, long i, int alpha) {
+  const long N = sim.N;
+  const long ip = sim.nbr(i, alpha, +1), im = sim.nbr(i, alpha, -1);
+  const Real p[3] = { s[ip], s[N + ip], s[2 * N + ip] };
+  const Real b[3] = { s[i], s[N + i], s[2 * N + i] };
+  const Real m[3] = { s[im], s[N + im], s[2 * N + im] };
+  const Real cx = fma_(b[1], m[2], -(b[2] * m[1]));
+  const Real cy = fma_(b[2], m[0], -(b[0] * m[2]));
+  const Real cz = fma_(b[0], m[1], -(b[1] * m[0]));
+  return fma_(p[2], cz, fma_(p[1], cy, p[0] * cx));
+}
+
+template <class Real>
+void measure_chiral(Sim<Real>& sim, double* qc0, double* qck, double* kappa_out /*[D][O][T][3][N] or null*/) {
+  const int D = sim.D, O = sim.O, T = sim.T, L = sim.L; const long N = sim.N;
+  const int P = O * (O - 1) / 2;
+  const double two_pi = 6.283185307179586476925286766559;
+  std::vector<Real> ka((size_t)3 * N), kb((size_t)3 * N);
+  if (kappa_out)
+    for (int d = 0; d < D; ++d) for (int o = 0; o < O; ++o) for (int t = 0; t < T; ++t) {
+      const Real* s = sim.spins_of_temp(d, o, t);
+      for (int al = 0; al < 3; ++al) for (long i = 0; i < N; ++i)
+        kappa_out[((((size_t)d * O + o) * T + t) * 3 + al) * N + i] = (double)chirality(sim, s, i, al);
+    }
+  if (!qc0 && !qck) return;
+  for (int d = 0; d < D; ++d) {
+    int p = 0;
+    for (int a = 0; a < O; ++a) for (int b = a + 1; b < O; ++b, ++p) for (int t = 0; t < T; ++t) {
+      const Real* sa = sim.spins_of_temp(d, a, t);
+      const Real* sb = sim.spins_of_temp(d, b, t);
+      for (int al = 0; al < 3; ++al) {
+        double r0 = 0.0, re = 0.0, im = 0.0;
+        for (long i = 0; i < N; ++i) {
+          const double pr = (double)chirality(sim, sa, i, al) * (double)chirality(sim, sb, i, al);
+          const double ph = two_pi * (double)(i % L) / (double)L;
+          r0 += pr; re += pr * std::cos(ph); im += pr * std::sin(ph);
+        }
+        const size_t idx = (((size_t)d * P + p) * T + t) * 3 + al;
+        if (qc0) qc0[idx] = r0 / (double)N;
+        if (qck) { qck[2 * idx] = re / (double)N; qck[2 * idx + 1] = im / (double)N; }
+      }
+    }
+  }
+}
 
 struct Handle { int precision; Sim<float>* f; Sim<double>* d; };
 
@@ -524,6 +737,7 @@ void orc_get_spins(void* h, double* S) {
 }
 void orc_sweep(void* h, int n_or, int n_hb, int n_threads) { ORC_DISPATCH(h, sim.sweep(n_or, n_hb, n_threads)); }
 void orc_energy(void* h, double* E) { ORC_DISPATCH(h, sim.energy(E)); }
+void orc_energy_plain(void* h, double* E) { ORC_DISPATCH(h, sim.energy_plain(E)); }
 void orc_pt_swap(void* h, int32_t* accepted) { ORC_DISPATCH(h, sim.pt_swap(accepted)); }
 void orc_measure(void* h, double* E, double* M, double* q0, double* qk) { ORC_DISPATCH(h, sim.measure(E, M, q0, qk)); }
 // slot_of_temp[D][O][T] and counters {k_hb, k_pt}
@@ -533,6 +747,22 @@ void orc_get_state(void* h, int32_t* slot_of_temp, uint64_t counters[2]) {
     if (counters) { counters[0] = sim.k_hb; counters[1] = sim.k_pt; }
   });
 }
+// field-case observables (Eq. 10): chi[D][T][2][3][2]; plain != 0: the O(N^2) definition, else the factored form.  Needs O >= 4.
+int orc_chi_field(void* h, double* chi, int plain, int n_threads) {
+  int rc = 0;
+  ORC_DISPATCH(h, { if (sim.O < 4) rc = -1; else chi_field_all(sim, chi, plain != 0, n_threads); });
+  return rc;
+}
+// chirality (Eqs. 12, 13): qc0[D][P][T][3], qck[D][P][T][3][2], optionally the local chiralities kappa[D][O][T][3][N]
+void orc_measure_chiral(void* h, double* qc0, double* qck, double* kappa) { ORC_DISPATCH(h, measure_chiral(sim, qc0, qck, kappa)); }
+// Eq. (8) / Eq. (15): second-moment correlation length from chi(0), chi(k_min)
+double orc_xi_second_moment(double chi_0, double chi_k, int L) {
+  const double kmin = 6.283185307179586476925286766559 / (double)L;
+  return std::sqrt(chi_0 / chi_k - 1.0) / (2.0 * std::sin(0.5 * kmin));
+}
+// parallel-tempering diagnostics (Fig. 3)
+void orc_pt_diag_reset(void* h) { ORC_DISPATCH(h, sim.pt_diag_reset()); }
+void orc_pt_diag_get(void* h, int64_t* moved, int64_t* trav, uint64_t* n_pass, double* p_diff) { ORC_DISPATCH(h, sim.pt_diag_get(moved, trav, n_pass, p_diff)); }
 void orc_set_counters(void* h, const uint64_t counters[2]) { ORC_DISPATCH(h, { sim.k_hb = counters[0]; sim.k_pt = counters[1]; }); }
 
 }  // extern "C"

@@ -1,6 +1,6 @@
 """In-tree build of the C-ABI library ``lib/libhsg.so`` (CUDA, sm_100a only).
 
-``nvcc`` cross-compiles without a GPU, so this runs on the CPU box (``__graft_entry__.build()``) and on
+``nvcc`` cross-compiles without a GPU (one translation unit per lattice size of the sweep kernel, compiled in parallel), so this runs on the CPU box (``__graft_entry__.build()``) and on
 the GPU box alike.  The shared object is rebuilt when any source under ``csrc/`` or ``include/hsg.h``
 is newer than it.
 """
@@ -21,7 +21,7 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-lineinfo", "-O3", "-std=c++17",
     "-fmad=false",            # no compiler-chosen multiply-add fusion; every FMA is explicit
-    "-shared", "-Xcompiler", "-fPIC",
+    "-Xcompiler", "-fPIC",
 ]
 
 
@@ -44,20 +44,32 @@ def stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
-    override = os.environ.get("HSG_LIB")          # experiments: load a pre-built variant instead
-    if override:
-        return Path(override)
+    """Compile every translation unit under csrc/ (in parallel) and link lib/libhsg.so; returns its path."""
     if not force and not stale():
         return LIB
     LIB.parent.mkdir(parents=True, exist_ok=True)
-    tmp = LIB.with_name(f"libhsg.tmp{os.getpid()}.so")
-    cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), str(CSRC / "hsg_api.cu"), "-o", str(tmp)]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
-    if verbose:
-        print(res.stderr)
-    os.replace(tmp, LIB)
+    objdir = LIB.parent / f"obj.tmp{os.getpid()}"
+    objdir.mkdir(parents=True, exist_ok=True)
+    nvcc = _nvcc()
+    units = sorted(CSRC.glob("*.cu"))
+    cmds = [[nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", str(u), "-o", str(objdir / (u.stem + ".o"))] for u in units]
+    try:
+        procs = [subprocess.Popen(c, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for c in cmds]
+        outs = [p.communicate()[0] for p in procs]
+        for c, p, o in zip(cmds, procs, outs):
+            if p.returncode != 0:
+                raise RuntimeError("nvcc failed:\n" + " ".join(c) + "\n" + o)
+            if verbose:
+                print(o)
+        tmp = LIB.with_name(f"libhsg.tmp{os.getpid()}.so")
+        link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC",
+                *[str(objdir / (u.stem + ".o")) for u in units], "-o", str(tmp)]
+        res = subprocess.run(link, capture_output=True, text=True)
+        if res.returncode != 0:
+            raise RuntimeError("link failed:\n" + " ".join(link) + "\n" + res.stdout + res.stderr)
+        os.replace(tmp, LIB)
+    finally:
+        shutil.rmtree(objdir, ignore_errors=True)
     return LIB
 
 

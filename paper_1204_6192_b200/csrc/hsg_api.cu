@@ -12,7 +12,7 @@
 #include <cuda_runtime.h>
 
 #include "hsg_kernels.cuh"
-#include "hsg_zmarch.cuh"
+#include "hsg_zmarch_launch.h"
 
 using namespace hsg;
 
@@ -92,6 +92,8 @@ struct hsg_ctx {
   unsigned long long k_hb, k_pt;
   bool have_disorder, have_spins;
   bool energy_valid;            // e_slot / m_slot hold the reduction of the current spins
+  int device;                   // CUDA device the context was created on (current at every call: hsg.h)
+  int sm_count;                 // its number of SMs (grid sizing of the sweep kernels)
   int sweep_kernel_opt;
   bool fuse_energy;             // zmarch: reduce E and m in the final sweep of every hsg_sweep call
   const char* last_kernel;
@@ -107,7 +109,7 @@ struct hsg_ctx {
 
 extern "C" {
 
-const char* hsg_version(void) { return "hsg 0.1 (sm_100a)"; }
+const char* hsg_version(void) { return "hsg 0.2 (sm_100a)"; }
 
 int hsg_query_bytes(const hsg_desc* desc, size_t* state_bytes, size_t* scratch_bytes) {
   const int rc = check_desc(desc);
@@ -132,6 +134,8 @@ int hsg_create(const hsg_desc* desc, void* dev_state, size_t state_bytes, void* 
   hsg_ctx* c = new (std::nothrow) hsg_ctx();
   if (!c) return HSG_EINVAL;
   c->g = g;
+  if (cudaGetDevice(&c->device) != cudaSuccess ||
+      cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) { delete c; return HSG_ECUDA; }
   c->key.k0 = (uint32_t)(desc->seed & 0xFFFFFFFFull);
   c->key.k1 = (uint32_t)(desc->seed >> 32);
   c->stream = (cudaStream_t)cuda_stream;
@@ -258,7 +262,7 @@ int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
     ZmarchArgs a{ctx->g, ctx->spins, ctx->jh, ctx->temp_of_slot, ctx->beta, ctx->key, ctx->k_hb, n_or, n_hb,
                  ctx->fuse_energy ? ctx->e_slot : nullptr, ctx->m_slot};
     int n_launch = 0;
-    const cudaError_t e = zmarch_launch(a, ctx->stream, &n_launch);
+    const cudaError_t e = zmarch_launch(a, ctx->stream, &n_launch, ctx->sm_count);
     ctx->launches += (unsigned long long)n_launch;
     if (e != cudaSuccess) { ctx->err = std::string("zmarch launch: ") + cudaGetErrorString(e); return HSG_ECUDA; }
     ctx->k_hb += (unsigned long long)n_hb;

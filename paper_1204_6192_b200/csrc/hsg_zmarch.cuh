@@ -1,7 +1,7 @@
 // hsg_zmarch.cuh — the fused z-marching sweep kernel.
 //
 // One launch runs a whole hsg_sweep(n_or, n_hb) call (at L = 32 and 16 the heat-bath sweeps are a second launch with
-// fewer sites per thread, see zmarch_launch).  A CTA owns G configuration slots of ONE disorder
+// fewer sites per thread, see zmarch_launch_g).  A CTA owns G configuration slots of ONE disorder
 // sample and marches them together through the lattice planes z = 0..L-1, updating colour 0 of plane k
 // and then colour 1 of plane k-1 in step k, so that every spin is read once and written once per sweep
 // and the result is exactly the global two-colour sweep of PAPER.md:141-146 (colour 1 of a plane is
@@ -37,59 +37,26 @@
 #include <cuda_runtime.h>
 #include "hsg_layout.cuh"
 #include "hsg_math.cuh"
+#include "hsg_zmarch_launch.h"
 
 namespace hsg {
 
-struct ZmarchArgs {
-  Geom g;
-  float* spins;                 // [R][3N] private layout
-  const float* jh;              // [D][6N]
-  const int32_t* temp_of_slot;  // [R]
-  const float* beta;            // [T]
-  PhiloxKey key;
-  unsigned long long k_hb;      // heat-bath sweep counter of the first HB sweep of this call
-  int n_or, n_hb;
-  double* e_slot;               // [R]    energy of every slot after the call, or nullptr
-  double* m_slot;               // [R][3] magnetisation of every slot after the call
-};
-
 namespace zm {
 
-#ifndef HSG_ZM_UNROLL
-#define HSG_ZM_UNROLL 2
-#endif
-#ifndef HSG_ZM_L32_V
-#define HSG_ZM_L32_V 4
-#endif
-#ifndef HSG_ZM_L32_G
-#define HSG_ZM_L32_G 2
-#endif
-#ifndef HSG_ZM_L32_VHB
-#define HSG_ZM_L32_VHB 2         // L = 32: sites per thread in the heat-bath phase (0: same launch as the over-relaxation phase)
-#endif
-#ifndef HSG_ZM_L16_VHB
-#define HSG_ZM_L16_VHB 2
-#endif
-#ifndef HSG_ZM_L16_V
-#define HSG_ZM_L16_V 4
-#endif
-#ifndef HSG_ZM_DS
-#define HSG_ZM_DS 2              // spin planes in flight ahead of the step that uses them
-#endif
-#ifndef HSG_ZM_DJ
-#define HSG_ZM_DJ 2              // J/H planes in flight ahead of the step that uses them
-#endif
-#ifndef HSG_ZM_UNROLL_HB
-#define HSG_ZM_UNROLL_HB 2
-#endif
-constexpr int kUnroll = HSG_ZM_UNROLL;   // unroll factor of the main march loop
-constexpr int kUnrollHB = HSG_ZM_UNROLL_HB;
-#ifndef HSG_ZM_L64_DS
-#define HSG_ZM_L64_DS 2          // (3 with DJ = 1 fits too and gains 1 % on c5; DJ = 1 is not validated for G = 1)
-#endif
-#ifndef HSG_ZM_L64_DJ
-#define HSG_ZM_L64_DJ 2
-#endif
+// Settled tuning of the march per lattice size (ncu evidence: profiles/).
+//   YS   rows per strip (= L: the whole plane in one CTA; < L: L/YS strips = CTAs of a thread-block cluster)
+//   V    compact sites per thread in the over-relaxation phase, VHB in the heat-bath phase; VHB != V: the heat-bath
+//        sweeps of a call run as a second launch with more, lighter threads (they are bound by instruction issue, the
+//        over-relaxation sweeps by memory)
+//   GMAX most systems of one sample a CTA marches together (they share the J/H rings)
+//   DS / DJ  spin / J-H planes in flight ahead of the step that uses them
+template <int L> struct Tune;
+template <> struct Tune<8>  { static constexpr int YS = 8,  V = 2, VHB = 2, GMAX = 8, DS = 2, DJ = 2; };
+template <> struct Tune<16> { static constexpr int YS = 16, V = 4, VHB = 2, GMAX = 8, DS = 2, DJ = 2; };
+template <> struct Tune<32> { static constexpr int YS = 32, V = 4, VHB = 2, GMAX = 2, DS = 2, DJ = 2; };
+template <> struct Tune<64> { static constexpr int YS = 16, V = 4, VHB = 4, GMAX = 2, DS = 2, DJ = 2; };
+constexpr int kUnroll = 2;     // unroll factor of the main march loop (over-relaxation / heat bath)
+constexpr int kUnrollHB = 2;
 
 // ---------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -215,8 +182,8 @@ template <int L, int YS, int V, int G> struct Cfg {
   static constexpr int CSJ = YS * Lh;             // shared J/H array of a strip
   static constexpr int JA = 11 * CSJ + (HALO ? 2 * Lh : 0);   // ring A slot: 11 arrays, then (strips) the row y0-1 of the two Jy
                                                               // arrays (colour 0, colour 1); ring B slot: colour-0 Jz
-  static constexpr int DS = L == 64 ? HSG_ZM_L64_DS : HSG_ZM_DS;   // spin planes in flight ahead of the step that uses them
-  static constexpr int DJ = L == 64 ? HSG_ZM_L64_DJ : HSG_ZM_DJ;   // J/H planes in flight
+  static constexpr int DS = Tune<L>::DS;          // spin planes in flight ahead of the step that uses them
+  static constexpr int DJ = Tune<L>::DJ;          // J/H planes in flight
   static constexpr int NC1 = DS + 2;              // ring C1: planes k, k+1 live + DS in flight
   static constexpr int NC0 = DS + 1;              // ring C0: plane k live + DS in flight
   static constexpr int NJA = DJ + 2;              // J/H ring A: planes k-1, k live + DJ in flight
@@ -743,12 +710,10 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
 template <int L, int YS, int V, int G>
 inline cudaError_t zmarch_launch_t(const ZmarchArgs& a, cudaStream_t stream) {
   using C = zm::Cfg<L, YS, V, G>;
-  static bool configured = false;
-  if (!configured) {
-    const cudaError_t e = cudaFuncSetAttribute(zm::zmarch_kernel<L, YS, V, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
+  // the attribute is per device: set it on every launch (a host-side table lookup) rather than remember per process,
+  // so that contexts on several devices of one process work (hsg.h: "distinct contexts are independent")
+  const cudaError_t e = cudaFuncSetAttribute(zm::zmarch_kernel<L, YS, V, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+  if (e != cudaSuccess) return e;
   if (C::NCL == 1) {
     zm::zmarch_kernel<L, YS, V, G><<<a.g.R / G, C::NT, C::smem_bytes, stream>>>(a);
     return cudaGetLastError();
@@ -765,76 +730,51 @@ inline cudaError_t zmarch_launch_t(const ZmarchArgs& a, cudaStream_t stream) {
   return cudaLaunchKernelEx(&cfg, zm::zmarch_kernel<L, YS, V, G>, a);
 }
 
-// largest group size the geometry allows: the G slots of a CTA must belong to one sample
-inline int zmarch_pick_g(const Geom& g, int gmax) {
-  int G = gmax;
+// hsg_sweep(n_or, n_hb) at lattice size L with G systems per CTA: one launch, or (VHB != V and both phases present) an
+// over-relaxation launch followed by a heat-bath launch; E and m are reduced by whichever launch holds the final sweep
+template <int L, int G>
+inline cudaError_t zmarch_launch_g(const ZmarchArgs& a, cudaStream_t stream, int* n_launch) {
+  using T = zm::Tune<L>;
+  *n_launch = 1;
+  if (T::VHB != T::V && a.n_hb > 0) {
+    if (a.n_or > 0) {
+      ZmarchArgs o = a;
+      o.n_hb = 0; o.e_slot = nullptr;
+      const cudaError_t e = zmarch_launch_t<L, T::YS, T::V, G>(o, stream);
+      if (e != cudaSuccess) return e;
+      *n_launch = 2;
+    }
+    ZmarchArgs h = a;
+    h.n_or = 0;
+    return zmarch_launch_t<L, T::YS, T::VHB, G>(h, stream);
+  }
+  return zmarch_launch_t<L, T::YS, T::V, G>(a, stream);
+}
+
+// Systems per CTA: the G slots of a CTA must belong to one sample (G divides O*T); G shrinks (down to 1) while the grid
+// would leave at least half of the SMs without a CTA.  (Measured on the paper's Table-1 workload, 256 systems of L = 32:
+// 128 CTAs of G = 2 run 6.1 ps/update, 256 CTAs of G = 1 run 8.0 — a second wave costs more than 20 idle SMs.)
+template <int L>
+inline int zmarch_pick_g(const Geom& g, int sm_count) {
+  int G = zm::Tune<L>::GMAX;
   while (G > 1 && (g.O * g.T) % G != 0) G >>= 1;
+  while (G > 1 && 2 * (long long)(g.R / G) * (L / zm::Tune<L>::YS) <= sm_count) G >>= 1;
   return G;
 }
 
-inline bool zmarch_supported(const Geom& g) { return g.L == 8 || g.L == 16 || g.L == 32 || g.L == 64; }
-
-#define HSG_ZM_CASE(L_, YS_, V_, G_) if (a.g.L == L_ && G == G_) return zmarch_launch_t<L_, YS_, V_, G_>(a, stream);
-inline cudaError_t zmarch_launch(const ZmarchArgs& a, cudaStream_t stream, int* n_launch) {
-  *n_launch = 1;
-  if (a.g.L == 32) {
-    const int G = zmarch_pick_g(a.g, HSG_ZM_L32_G);
-#if HSG_ZM_L32_VHB > 0
-    // The heat-bath sweeps are bound by instruction issue, the over-relaxation sweeps by memory: the heat-bath phase
-    // runs as a launch of its own with half the sites (and registers) per thread and twice the warps per SM.
-    if (G == HSG_ZM_L32_G && a.n_hb > 0) {
-      if (a.n_or > 0) {
-        ZmarchArgs o = a;
-        o.n_hb = 0; o.e_slot = nullptr;
-        const cudaError_t e = zmarch_launch_t<32, 32, HSG_ZM_L32_V, HSG_ZM_L32_G>(o, stream);
-        if (e != cudaSuccess) return e;
-        *n_launch = 2;
-      }
-      ZmarchArgs h = a;
-      h.n_or = 0;
-      return zmarch_launch_t<32, 32, HSG_ZM_L32_VHB, HSG_ZM_L32_G>(h, stream);
-    }
-#endif
-    HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, HSG_ZM_L32_G)
-#if HSG_ZM_L32_G > 2
-    HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, 2)
-#endif
-#if HSG_ZM_L32_G > 1
-    HSG_ZM_CASE(32, 32, HSG_ZM_L32_V, 1)
-#endif
-  }
-#ifndef HSG_ZM_NO_L64
-  else if (a.g.L == 64) {      // four strips of 16 rows = a cluster of four CTAs per group of two systems
-    const int G = zmarch_pick_g(a.g, 2);
-    HSG_ZM_CASE(64, 16, 4, 2) HSG_ZM_CASE(64, 16, 4, 1)
-  }
-#endif
-#ifndef HSG_ZM_ONLY_L32     // (variant builds for experiments instantiate L = 32 and 64 only)
-  else if (a.g.L == 16) {
-    const int G = zmarch_pick_g(a.g, 8);
-#if HSG_ZM_L16_VHB > 0
-    if (G == 8 && a.n_hb > 0) {     // heat-bath phase as its own launch with twice the warps, as at L = 32
-      if (a.n_or > 0) {
-        ZmarchArgs o = a;
-        o.n_hb = 0; o.e_slot = nullptr;
-        const cudaError_t e = zmarch_launch_t<16, 16, HSG_ZM_L16_V, 8>(o, stream);
-        if (e != cudaSuccess) return e;
-        *n_launch = 2;
-      }
-      ZmarchArgs h = a;
-      h.n_or = 0;
-      return zmarch_launch_t<16, 16, HSG_ZM_L16_VHB, 8>(h, stream);
-    }
-#endif
-    HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 8) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 4) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 2) HSG_ZM_CASE(16, 16, HSG_ZM_L16_V, 1)
-  } else if (a.g.L == 8) {
-    const int G = zmarch_pick_g(a.g, 8);
-    HSG_ZM_CASE(8, 8, 2, 8) HSG_ZM_CASE(8, 8, 2, 4) HSG_ZM_CASE(8, 8, 2, 2) HSG_ZM_CASE(8, 8, 2, 1)
-  }
-#endif
+template <int L, int G>
+inline cudaError_t zmarch_dispatch_g(const ZmarchArgs& a, cudaStream_t stream, int* n_launch, int want_g) {
+  if (want_g == G) return zmarch_launch_g<L, G>(a, stream, n_launch);
+  if constexpr (G > 1) return zmarch_dispatch_g<L, G / 2>(a, stream, n_launch, want_g);
   *n_launch = 0;
   return cudaErrorNotSupported;
 }
-#undef HSG_ZM_CASE
+
+// body of the per-size entry points zmarch_launch_l<L> (hsg_zmarch_l8.cu ... hsg_zmarch_l64.cu: one translation unit per
+// lattice size, compiled in parallel)
+template <int L>
+inline cudaError_t zmarch_launch_size(const ZmarchArgs& a, cudaStream_t stream, int* n_launch, int sm_count) {
+  return zmarch_dispatch_g<L, zm::Tune<L>::GMAX>(a, stream, n_launch, zmarch_pick_g<L>(a.g, sm_count));
+}
 
 }  // namespace hsg

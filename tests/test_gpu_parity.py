@@ -9,6 +9,7 @@ import pytest
 
 import hsg_inputs
 import oracle
+from tests.pt_band import excuse_or_fail
 
 pytestmark = pytest.mark.gpu
 
@@ -34,6 +35,24 @@ def _pair(L, D, O, T, seed, h_r=0.1, t_min=0.08, t_max=0.30, kernel="generic", s
 
 def _spins(eng):
     return eng.get_spins().cpu().numpy().astype(np.float64)
+
+
+def _check_energy(E_gpu, orc, idx=None):
+    """Every GPU energy is checked twice: (i) against the oracle's energy() — the PAPER.md:185 reading the
+    parallel-tempering decisions use (single-precision site terms, fp64 sum), where only the order of the
+    fp64 additions may differ: rtol 1e-12; (ii) against the oracle's energy_plain() — Eq. (1) as written, forward bonds
+    once, all fp64 — inside the derived bound N/2 * 9 * 2^-24 * 8 (and BASELINE.json's relative 1e-5 per spin)."""
+    E_o, E_p = np.asarray(orc.energy()), np.asarray(orc.energy_plain())
+    if idx is not None:
+        E_o, E_p = E_o[idx], E_p[idx]
+    E_gpu = np.asarray(E_gpu).reshape(E_o.shape)
+    N = orc.N
+    np.testing.assert_allclose(E_gpu, E_o, rtol=1e-12, atol=0)
+    assert np.abs(E_gpu - E_p).max() < N / 2 * 9 * 2.0**-24 * 8
+    # BASELINE.json: energy per spin, relative difference <= 1e-5.  Hot systems have e = E/N ~ 0 (north_star: "energy is zero
+    # at beta = 0"), where a relative difference means nothing: below |e| = 1e-3 the difference is taken relative to 1e-3.
+    e_g, e_p = E_gpu / N, E_p / N
+    assert (np.abs(e_g - e_p) <= 1e-5 * np.maximum(np.abs(e_p), 1e-3)).all()
 
 
 @pytest.mark.parametrize("L,D,O,T", [(4, 2, 2, 3), (6, 1, 1, 2), (8, 1, 2, 16), (10, 2, 1, 3), (12, 1, 2, 2), (16, 3, 2, 4)])
@@ -69,10 +88,12 @@ def test_hb_sweeps_bit_exact(kernel, L, D, O, T):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-@pytest.mark.parametrize("cfg,D", [("c1", 1), ("c2", 2), ("c3", 2), ("c4", 1), ("c5", 1)])
-def test_ten_sweeps_of_the_baseline_configs(kernel, cfg, D):
-    """BASELINE.json: per-component spin difference <= 1e-4 after 10 sweeps (cold start, OR then HB)."""
-    c, temps, J, H = hsg_inputs.make_config(cfg, n_samples=D)
+@pytest.mark.parametrize("cfg,D,h_r", [("c1", 1, None), ("c2", 2, None), ("c3", 2, 0.05), ("c3", 2, 0.1), ("c3", 2, 0.2), ("c4", 1, None),
+                                       ("c5", 1, None), ("t1", 1, None)])
+def test_ten_sweeps_of_the_baseline_configs(kernel, cfg, D, h_r):
+    """BASELINE.json: per-component spin difference <= 1e-4 after 10 sweeps (cold start, OR then HB).  c3 at every field
+    strength of its scan; t1 = the paper's Table-1 workload (T = 100: beta|h| ~ 0.02), one sample."""
+    c, temps, J, H = hsg_inputs.make_config(cfg, n_samples=D, h_r=h_r)
     import paper_1204_6192_b200 as hsg
     try:
         eng = hsg.hsg_create(c["L"], D, c["n_replicas"], temps, c["seed"], kernel=kernel)
@@ -87,11 +108,47 @@ def test_ten_sweeps_of_the_baseline_configs(kernel, cfg, D):
     assert np.abs(a - b).max() <= 1e-4
     assert np.abs(a - b).max() == 0.0
     N = c["L"] ** 3
-    e_gpu = eng.energy().cpu().numpy() / N
-    e_orc = orc.energy() / N
-    assert np.abs(e_gpu / e_orc - 1.0).max() <= 1e-5
-    np.testing.assert_allclose(e_gpu, e_orc, rtol=1e-12, atol=0)
+    _check_energy(eng.energy().cpu().numpy(), orc)
     assert np.abs(np.sqrt((a.reshape(D, -1, 3, N) ** 2).sum(axis=2)) - 1).max() < 1e-4   # still unit vectors
+
+
+HOT_LADDERS = {
+    "t100_1e5_1e29": [1e2, 1e5, 1e29, 1e30],                 # a = beta|h| ~ 2e-2 (Table 1), ~2e-5 (series branch), ~0
+    "straddle_1e-4": [1e2, 1e4, 2e4, 3e4, 1e5, 1e29],         # a crosses the 1e-4 switch between the series and the inverse CDF
+}
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("L", [8, 32])
+@pytest.mark.parametrize("ladder", sorted(HOT_LADDERS))
+def test_hot_ladders_reach_the_small_a_branches_bit_exact(kernel, L, ladder):
+    """Heat bath at high temperature: 0 < a < 1e-4 takes the series t = 2v(1 - a u1), a ~ 0.02 is the
+    paper's Table-1 regime, T = 1e29 is beta -> 0.  Both kernels, L = 8 and 32, bit for bit; the test also
+    checks that the ladder really put sites on both sides of the switch."""
+    import paper_1204_6192_b200 as hsg
+    temps = np.asarray(HOT_LADDERS[ladder], dtype=np.float32)
+    D, O, T, seed = 1, 2, len(temps), 61
+    J = hsg_inputs.couplings(L, D, seed); H = hsg_inputs.gaussian_field(L, D, 0.1, seed)
+    eng = hsg.hsg_create(L, D, O, temps, seed, kernel=kernel)
+    orc = oracle.Oracle(L, D, O, temps, seed, precision=32, n_threads=8)
+    eng.set_disorder(J, H); orc.set_disorder(J, H)
+    eng.init_spins(); orc.init_spins()
+    # which branch do the sites take?  a = beta |h| with |h| of the start configuration (numpy, fp64: only a census)
+    S0 = orc.get_spins()[0]                                       # [O][T][3][z][y][x]
+    hJ = np.zeros_like(S0)
+    for d, ax in enumerate((5, 4, 3)):
+        hJ += J[0, d][None, None, None] * np.roll(S0, -1, axis=ax) + np.roll(J[0, d], 1, axis=ax - 3)[None, None, None] * np.roll(S0, 1, axis=ax)
+    a = np.linalg.norm(hJ + H[0][None, None], axis=2) / temps.astype(np.float64)[None, :, None, None, None]
+    assert (a < 1e-4).any() and (a[a > 0] < 1e-4).any() and (a > 1e-4).any()
+    if ladder == "straddle_1e-4":
+        mid = a[:, 1:4]
+        assert (mid < 1e-4).any() and (mid > 1e-4).any()         # the switch is crossed inside single systems
+    for _ in range(2):
+        eng.sweep(2, 2); orc.sweep(2, 2)
+    assert eng.last_sweep_kernel() == kernel
+    assert np.abs(_spins(eng) - orc.get_spins()).max() == 0.0
+    _check_energy(eng.energy().cpu().numpy(), orc)
+    assert np.array_equal(eng.pt_swap().cpu().numpy(), orc.pt_swap())
 
 
 def test_energy_and_measurements_match_oracle():
@@ -100,7 +157,7 @@ def test_energy_and_measurements_match_oracle():
     eng.sweep(2, 2); orc.sweep(2, 2)
     E, M, q0, qk = (x.cpu().numpy() for x in eng.measure())
     Eo, Mo, q0o, qko = orc.measure()
-    np.testing.assert_allclose(E, Eo, rtol=1e-12)
+    _check_energy(E, orc)
     np.testing.assert_allclose(M, Mo, rtol=0, atol=1e-13)
     np.testing.assert_allclose(q0, q0o, rtol=0, atol=1e-13)
     np.testing.assert_allclose(qk, qko, rtol=0, atol=1e-13)
@@ -108,12 +165,12 @@ def test_energy_and_measurements_match_oracle():
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-def test_lockstep_steps_pt_decisions_and_observables(kernel):
-    """c1 (L=8, 1 x 2 x 16): 40 full steps (5 OR + 1 HB + PT) in lockstep; decisions must be identical except
-    inside the 1e-4 band around the acceptance threshold (BASELINE.json)."""
+def test_lockstep_c1_all_1000_steps_pt_decisions_and_observables(kernel):
+    """c1 as BASELINE.json states it (L=8, 1 x 2 x 16, 5 OR + 1 HB + PT, 1000 steps, seed 1) in lockstep: spins every
+    step (<= 1e-4; in fact identical), every swap decision (a difference is excused only if THAT pair was inside the 1e-4
+    band, see _excuse_or_fail), permutation and, every 50 steps, E / m / q(0) / q(k_min)."""
     c, temps, J, H = hsg_inputs.make_config("c1")
     import paper_1204_6192_b200 as hsg
-    from tests import philox_np as pnp
     try:
         eng = hsg.hsg_create(c["L"], 1, 2, temps, c["seed"], kernel=kernel)
     except hsg.HsgError as e:
@@ -122,32 +179,59 @@ def test_lockstep_steps_pt_decisions_and_observables(kernel):
     orc = oracle.Oracle(c["L"], 1, 2, temps, c["seed"], precision=32)
     orc.set_disorder(J, H); orc.init_spins()
     beta = (1.0 / temps.astype(np.float64)).astype(np.float32).astype(np.float64)
-    n_acc = 0
-    for step in range(40):
-        eng.sweep(5, 1); orc.sweep(5, 1)
-        Eo = orc.energy()
+    n_acc, n_steps = 0, c["steps"]
+    assert n_steps == 1000
+    for step in range(n_steps):
+        eng.sweep(c["n_or"], c["n_hb"]); orc.sweep(c["n_or"], c["n_hb"])
+        E_pre = orc.energy()
         acc_o = orc.pt_swap()
         acc_g = eng.pt_swap().cpu().numpy()
-        if not np.array_equal(acc_g, acc_o):        # excuse only decisions inside the band
-            for (d, o, t) in zip(*np.nonzero(acc_g != acc_o)):
-                u = pnp.u01(pnp.draw(pnp.DOMAIN_PT, t, step, d * 2 + o, c["seed"])[0])
-                # energies of the pair as the walk up the ladder saw them are not reconstructed here:
-                # a disagreement is only tolerated at all if some pair of this chain is within the band
-                x = (beta[1:] - beta[:-1]) * (Eo[d, o, 1:] - Eo[d, o, :-1])
-                assert np.abs(x - np.log(u)).min() < 1e-4
-            orc_perm = orc.get_state()[0]
-            eng.set_state(perm=orc_perm)
+        if not np.array_equal(acc_g, acc_o):
+            excuse_or_fail(acc_g, acc_o, E_pre, beta, c["seed"], step, 2)
+            eng.set_state(perm=orc.get_state()[0])
         n_acc += int(acc_o.sum())
-        perm_g = eng.get_state()[0].cpu().numpy()
-        assert np.array_equal(perm_g, orc.get_state()[0])
+        assert np.array_equal(eng.get_state()[0].cpu().numpy(), orc.get_state()[0])
         assert np.abs(_spins(eng) - orc.get_spins()).max() <= 1e-4
+        if step % 50 == 49:
+            E, M, q0, qk = (x.cpu().numpy() for x in eng.measure())
+            Eo, Mo, q0o, qko = orc.measure()
+            _check_energy(E, orc)
+            np.testing.assert_allclose(M, Mo, atol=1e-13)
+            np.testing.assert_allclose(q0, q0o, atol=1e-12)
+            np.testing.assert_allclose(qk, qko, atol=1e-12)
     assert n_acc > 0
-    E, M, q0, qk = (x.cpu().numpy() for x in eng.measure())
-    Eo, Mo, q0o, qko = orc.measure()
-    assert np.abs(E / Eo - 1).max() <= 1e-5
-    np.testing.assert_allclose(q0, q0o, atol=1e-12)
-    np.testing.assert_allclose(qk, qko, atol=1e-12)
-    assert eng.get_state()[1] == (40, 40)
+    assert np.abs(_spins(eng) - orc.get_spins()).max() == 0.0
+    assert eng.get_state()[1] == (n_steps, n_steps)
+
+
+@pytest.mark.parametrize("h_r", [0.05, 0.2])
+def test_lockstep_c3_measure_every_step(h_r):
+    """c3's shape (L=16, 2 replicas x 24 temperatures in [0.06, 0.25], field scan, measure EVERY step): 20 steps in
+    lockstep on two disorder samples, comparing E, m, q(0), q(k_min), the swap decisions and the spins each step."""
+    import paper_1204_6192_b200 as hsg
+    D = 2
+    c, temps, J, H = hsg_inputs.make_config("c3", n_samples=D, h_r=h_r)
+    L, O, T = c["L"], c["n_replicas"], len(temps)
+    eng = hsg.hsg_create(L, D, O, temps, c["seed"])
+    orc = oracle.Oracle(L, D, O, temps, c["seed"], precision=32, n_threads=8)
+    eng.set_disorder(J, H); orc.set_disorder(J, H)
+    eng.init_spins(); orc.init_spins()
+    beta = (1.0 / temps.astype(np.float64)).astype(np.float32).astype(np.float64)
+    for step in range(20):
+        eng.sweep(c["n_or"], c["n_hb"]); orc.sweep(c["n_or"], c["n_hb"])
+        E_pre = orc.energy()
+        acc_o = orc.pt_swap(); acc_g = eng.pt_swap().cpu().numpy()
+        if not np.array_equal(acc_g, acc_o):
+            excuse_or_fail(acc_g, acc_o, E_pre, beta, c["seed"], step, O)
+            eng.set_state(perm=orc.get_state()[0])
+        E, M, q0, qk = (x.cpu().numpy() for x in eng.measure())
+        Eo, Mo, q0o, qko = orc.measure()
+        _check_energy(E, orc)
+        np.testing.assert_allclose(M, Mo, rtol=0, atol=1e-13)
+        np.testing.assert_allclose(q0, np.asarray(q0o).reshape(q0.shape), rtol=0, atol=1e-12)
+        np.testing.assert_allclose(qk, np.asarray(qko).reshape(qk.shape), rtol=0, atol=1e-12)
+        assert np.abs(_spins(eng) - orc.get_spins()).max() == 0.0
+    assert eng.last_sweep_kernel() == "zmarch"
 
 
 def test_set_get_spins_roundtrip_and_checkpoint():
@@ -256,7 +340,7 @@ def test_energy_fused_into_the_last_sweep_matches_oracle_and_the_separate_reduct
                                                                                  eng._new((D, O, T, 3), eng.torch.float64), None, None)))
     assert eng.launch_count() - n0 == 2                  # two gathers, no reduction pass over the spins
     Eo, Mo, _, _ = orc.measure()
-    np.testing.assert_allclose(E, Eo, rtol=1e-12)
+    _check_energy(E, orc)
     np.testing.assert_allclose(M, Mo, rtol=0, atol=1e-13)
     eng.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
     eng.sweep(0, 0)                                      # no-op; cached values stay valid
@@ -296,8 +380,7 @@ def test_full_size_configs_on_sampled_disorder_samples(cfg, samples):
         b = orc.get_spins()[0]
         assert np.abs(a - b).max() == 0.0, f"{cfg} sample {d}: spins"
         Eo, Mo, q0o, qko = orc.measure()
-        np.testing.assert_allclose(E[d], np.asarray(Eo)[0], rtol=1e-12)
-        assert np.abs(E[d] / np.asarray(Eo)[0] - 1).max() <= 1e-5
+        _check_energy(E[d], orc, idx=0)
         np.testing.assert_allclose(M[d], np.asarray(Mo).reshape(M[d].shape), rtol=0, atol=1e-13)
         np.testing.assert_allclose(q0[d], np.asarray(q0o).reshape(q0[d].shape), rtol=0, atol=1e-12)
         np.testing.assert_allclose(qk[d], np.asarray(qko).reshape(qk[d].shape), rtol=0, atol=1e-12)
@@ -340,6 +423,5 @@ def test_equilibrium_energy_and_q2_agree_over_64_samples():
     for name, a, b in (("e", e_i, e_o), ("q2", q_i, q_o)):
         diff = a - b                                                  # [D][T], paired by disorder sample
         mean, sem = diff.mean(axis=0), diff.std(axis=0, ddof=1) / np.sqrt(D)
-        assert (np.abs(mean) < 3.0 * sem + 1e-12).sum() >= T - 1, (name, mean / sem)   # 3 sigma at (at least) 7 of 8 temperatures
-        assert np.abs(mean / sem).max() < 4.5, (name, mean / sem)
+        assert (np.abs(mean) < 3.0 * sem + 1e-12).all(), (name, mean / sem)              # within 3 sigma at every temperature
     assert (e_o[:, 0] < e_o[:, -1]).all() and (q_o[:, 0].mean() > q_o[:, -1].mean())   # colder: lower energy, larger overlap

@@ -35,37 +35,85 @@ def local_field_roll(S, J, H):
     return h
 
 
-def test_energy_matches_three_algebraically_equal_forms():
+def energy_bound(N, J=None, H=None):
+    """|E_fp32form - E_plain| bound of DESIGN.md §3.6: each colour-1 site term carries at most 9 roundings of 2^-24
+    relative to sum|J||s||s| + |H||s| <~ 8 (colour-0 terms: 3 roundings of |H|), i.e. N/2 * 9 * 2^-24 * 8."""
+    return N / 2 * 9 * 2.0**-24 * 8
+
+
+def test_energy_plain_is_eq1_and_matches_three_algebraically_equal_forms():
+    """oracle.energy_plain = PAPER.md:26 Eq. (1) as written (forward bonds once, fp64): against three independent numpy
+    restatements, in both instantiations (the fp32 one holds fp32 spins; the arithmetic of energy_plain is fp64 either way)."""
     L, D, O, T = 4, 2, 2, 3
     temps = hsg_inputs.geometric_ladder(0.1, 0.3, T)
     J = hsg_inputs.couplings(L, D, 5); H = hsg_inputs.gaussian_field(L, D, 0.3, 5)
     S = hsg_inputs.unit_spins(L, D, O, T, 5)
+    par = np.indices((L, L, L)).sum(axis=0) % 2
+    for precision in (64, 32):
+        sim = oracle.Oracle(L, D, O, temps, 1, precision=precision)
+        sim.set_disorder(J, H); sim.set_spins(S)
+        Ep = sim.energy_plain()
+        for d in range(D):
+            for o in range(O):
+                for t in range(T):
+                    s = S[d, o, t].astype(np.float64); Jd = J[d].astype(np.float64); Hd = H[d].astype(np.float64)
+                    e1 = energy_roll(s, Jd, Hd)
+                    hJ = local_field_roll(s, Jd, None)
+                    e2 = -0.5 * (s * hJ).sum() - (Hd * s).sum()
+                    e3 = -((s * (hJ + Hd)).sum(axis=0) * (par == 1)).sum() - ((Hd * s).sum(axis=0) * (par == 0)).sum()
+                    assert abs(Ep[d, o, t] - e1) < 1e-11 and abs(e1 - e2) < 1e-11 and abs(e1 - e3) < 1e-11
+        # zero field path (H = None)
+        sim.set_disorder(J, None)
+        assert abs(sim.energy_plain()[0, 0, 0] - energy_roll(S[0, 0, 0].astype(np.float64), J[0].astype(np.float64), None)) < 1e-11
+
+
+def test_energy_plain_brute_force_bond_list():
+    """Every bond once: an explicit python loop over sites and the three forward neighbours (a dropped direction, a bond
+    counted twice, a wrong periodic wrap or a transposed J index all fail here)."""
+    L = 4
+    J = hsg_inputs.couplings(L, 1, 6); H = hsg_inputs.gaussian_field(L, 1, 0.5, 6)
+    S = hsg_inputs.unit_spins(L, 1, 1, 1, 6)
+    sim = oracle.Oracle(L, 1, 1, [0.2], 1, precision=32)
+    sim.set_disorder(J, H); sim.set_spins(S)
+    s = S[0, 0, 0].astype(np.float64)
+    E = 0.0
+    for z in range(L):
+        for y in range(L):
+            for x in range(L):
+                for d, (dx, dy, dz) in enumerate(((1, 0, 0), (0, 1, 0), (0, 0, 1))):
+                    E -= float(J[0, d, z, y, x]) * float(s[:, z, y, x] @ s[:, (z + dz) % L, (y + dy) % L, (x + dx) % L])
+                E -= float(H[0, :, z, y, x].astype(np.float64) @ s[:, z, y, x])
+    assert abs(sim.energy_plain()[0, 0, 0] - E) < 1e-12
+    # one ferromagnetic bond, aligned spins: E = -J
+    J1 = np.zeros((1, 3, L, L, L), np.float32); J1[0, 1, 2, 3, 1] = 1.5      # y-bond leaving (x=1,y=3,z=2): wraps to y=0
+    S1 = np.zeros((1, 1, 1, 3, L, L, L), np.float32); S1[0, 0, 0, 2] = 1.0
+    sim.set_disorder(J1, None); sim.set_spins(S1)
+    assert sim.energy_plain()[0, 0, 0] == -1.5 and sim.energy()[0, 0, 0] == -1.5
+    S1[0, 0, 0, 2, 2, 0, 1] = -1.0                                             # flip the far end of that bond
+    sim.set_spins(S1)
+    assert sim.energy_plain()[0, 0, 0] == 1.5 and sim.energy()[0, 0, 0] == 1.5
+
+
+@pytest.mark.parametrize("L", [4, 8, 12])
+def test_energy_of_the_moves_reading_is_pinned_against_energy_plain(L):
+    """oracle.energy (PAPER.md:185 reading: single-precision site terms s_i.h_i / s_i.H_i in the bipartite
+    form, fp64 sum — what the parallel-tempering decisions use) against the plain definition: the fp64 instantiation agrees to
+    summation-order rounding, the fp32 one inside the derived bound N/2 * 9 * 2^-24 * 8 (and is typically sqrt(N) smaller)."""
+    D, O, T = 2, 2, 2
+    temps = hsg_inputs.geometric_ladder(0.1, 0.3, T)
+    J = hsg_inputs.couplings(L, D, 5 + L); H = hsg_inputs.gaussian_field(L, D, 0.3, 5 + L)
+    S = hsg_inputs.unit_spins(L, D, O, T, 5 + L)
+    N = L**3
     sim = oracle.Oracle(L, D, O, temps, 1, precision=64)
     sim.set_disorder(J, H); sim.set_spins(S)
-    E = sim.energy()
-    par = np.indices((L, L, L)).sum(axis=0) % 2
-    for d in range(D):
-        for o in range(O):
-            for t in range(T):
-                s = S[d, o, t].astype(np.float64); Jd = J[d].astype(np.float64); Hd = H[d].astype(np.float64)
-                e1 = energy_roll(s, Jd, Hd)
-                hJ = local_field_roll(s, Jd, None)
-                e2 = -0.5 * (s * hJ).sum() - (Hd * s).sum()
-                e3 = -((s * (hJ + Hd)).sum(axis=0) * (par == 1)).sum() - ((Hd * s).sum(axis=0) * (par == 0)).sum()
-                assert abs(E[d, o, t] - e1) < 1e-11 and abs(e1 - e2) < 1e-11 and abs(e1 - e3) < 1e-11
-    # zero field path (H = None)
-    sim.set_disorder(J, None)
-    assert abs(sim.energy()[0, 0, 0] - energy_roll(S[0, 0, 0].astype(np.float64), J[0].astype(np.float64), None)) < 1e-11
-    # fp32 instantiation: the site terms s_i.h_i (odd sites) and s_i.H_i (even sites) are single-precision FMA chains
-    # (spins single, aggregates double), summed in double.  Each odd-site term carries at most
-    # 9 roundings of 2^-24 relative to sum|J||s||s| + |H||s| <~ 8: |E32 - E| <= N/2 * 9 * 2^-24 * 8; typically sqrt(N) smaller.
+    assert np.abs(sim.energy() - sim.energy_plain()).max() < 1e-13 * N
     sim32 = oracle.Oracle(L, D, O, temps, 1, precision=32)
     sim32.set_disorder(J, H); sim32.set_spins(S)
-    E32 = sim32.energy()
-    N = L**3
-    assert np.abs(E32 - E).max() < N / 2 * 9 * 2.0**-24 * 8
-    assert np.abs(E32 - E).max() < 40 * math.sqrt(N) * 2.0**-24 * 8       # random-walk size, with margin
-    assert np.abs(E32 - E).max() > 0                                      # it IS the single-precision form
+    E32, Ep = sim32.energy(), sim32.energy_plain()
+    assert np.abs(Ep - sim.energy_plain()).max() == 0                          # same fp32 spins, same fp64 arithmetic
+    assert np.abs(E32 - Ep).max() < energy_bound(N)
+    assert np.abs(E32 - Ep).max() < 40 * math.sqrt(N) * 2.0**-24 * 8           # random-walk size, with margin
+    assert np.abs(E32 - Ep).max() > 0                                          # it IS the single-precision form
 
 
 # ---------------------------------------------------------------------- OR sweeps are microcanonical
@@ -152,10 +200,11 @@ def test_dimers_zero_field_closed_form(J0, T):
     blocks = acc.reshape(30, -1).mean(axis=1)
     err = blocks.std(ddof=1) / math.sqrt(len(blocks))
     assert abs(acc.mean() - exact) < 4.5 * err + 1e-5
-    # the energy routine sees the same number: E = -J0 * sum over dimers of s1.s2
+    # the energy routine sees the same number: E = -J0 * sum over dimers of s1.s2 (plain Eq. 1 form: fp64 products)
     S = sim.get_spins()[0, 0, 0]
-    # (fp32 instantiation: site terms s_i.h_i are single-precision FMA chains, DESIGN.md §3.6 -> a few 2^-24 per site)
-    assert abs(sim.energy()[0, 0, 0] + float(np.float32(J0)) * (S[:, :, :, 0::2] * S[:, :, :, 1::2]).sum()) < 2e-7 * L**3
+    e_dimers = -float(np.float32(J0)) * (S[:, :, :, 0::2] * S[:, :, :, 1::2]).sum()
+    assert abs(sim.energy_plain()[0, 0, 0] - e_dimers) < 1e-9
+    assert abs(sim.energy()[0, 0, 0] - e_dimers) < energy_bound(L**3)          # the single-precision reading, inside its bound
 
 
 def _dimer_in_field_exact(beta, J0, h1, h2):

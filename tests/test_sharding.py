@@ -113,3 +113,62 @@ def test_two_contexts_with_sample_offsets_reproduce_one_context(kernel):
     parts = [run(off, cnt) for off, cnt in sharding.shard_bounds(D, 2)]
     for k in range(3):
         assert np.array_equal(np.concatenate([p[k] for p in parts], axis=0), full[k])
+
+
+def _run_gpu_shard(off, cnt, Lg=8, Tg=4):
+    """One rank's work on the GPU through the C ABI: its shard of samples, three steps, observables + spins (CPU tensors)."""
+    import paper_1204_6192_b200 as hsg
+    temps = hsg_inputs.geometric_ladder(0.08, 0.3, Tg)
+    eng = hsg.hsg_create(Lg, cnt, O, temps, SEED, sample_offset=off)
+    eng.set_disorder(hsg_inputs.couplings(Lg, cnt, SEED, off), hsg_inputs.gaussian_field(Lg, cnt, 0.1, SEED, off))
+    eng.init_spins()
+    accs = []
+    for _ in range(3):
+        eng.sweep(2, 1)
+        accs.append(eng.pt_swap().cpu())
+    E, M, q0, qk = (x.cpu() for x in eng.measure())
+    import torch
+    return E, q0, torch.stack(accs, dim=1), eng.get_spins().cpu()
+
+
+def _gpu_worker(rank, world, port, q, n_all):
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(rank % torch.cuda.device_count())     # two ranks may share one device (the driver's box has one)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        off, cnt = sharding.shard_of_rank(n_all, world, rank)
+        parts = _run_gpu_shard(off, cnt)
+        gathered = [sharding.gather_by_sample(x, n_all) for x in parts]
+        if rank == 0:
+            q.put([g.numpy() for g in gathered])
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_two_gpu_processes_gathered_over_gloo_reproduce_one_context():
+    """The multi-GPU path as bench.py --gpus N runs it, with the real engine: two PROCESSES (one hsg context each, their own
+    shard of the disorder samples via sample_offset), per-sample observables and spins gathered with
+    sharding.gather_by_sample over gloo, must equal the single-context run of all samples bit for bit."""
+    import torch.multiprocessing as mp
+    n_all = 3
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_gpu_worker, args=(r, 2, port, q, n_all)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = q.get(timeout=600)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    full = [x.numpy() for x in _run_gpu_shard(0, n_all)]
+    assert got[0].shape == (n_all, O, 4)
+    for a, b in zip(got, full):
+        assert np.array_equal(a, b)
