@@ -48,15 +48,17 @@ def _peaks():
 
 
 def _traffic(workload, kernel):
-    """dram bytes per sweep-kernel launch from the committed ncu capture (profiles/traffic.csv), or None."""
+    """(dram bytes per sweep-kernel launch, where the number comes from) from the committed ncu capture listed in
+    profiles/traffic.csv (`workload:kernel,bytes,capture`), or (None, why)."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         for line in open(p):
             if line.startswith(f"{workload}:{kernel},"):
-                return float(line.strip().split(",")[1])
+                f = line.strip().split(",")
+                return float(f[1]), f"profiles/traffic.csv: {f[2] if len(f) > 2 else 'ncu --set full capture'} (not re-measured in this run)"
     except Exception:
         pass
-    return None
+    return None, "no ncu capture of this workload in profiles/traffic.csv"
 
 
 class ClockSampler:
@@ -197,48 +199,82 @@ def main_ours(args, cfg, temps):
     for _ in range(args.warmup):
         step()
     barrier()
-    # hsg_sweep(n_or, n_hb) is one launch, or (L = 32) an over-relaxation launch followed by a heat-bath launch; in
-    # that case the timed loop makes the same two launches through two calls so that each can be timed on its own
     n0 = eng.launch_count(); eng.sweep(n_or, n_hb); sweep_launches_per_call = eng.launch_count() - n0
     kernel = eng.last_sweep_kernel()
     two_phase = kernel == "zmarch" and sweep_launches_per_call == 2 and n_or > 0 and n_hb > 0
     eng.pt_swap(out=acc)
     barrier()
+
+    # ---- the timed region: EXACTLY args.steps steps of the product calls (hsg_sweep(n_or, n_hb), hsg_pt_swap, hsg_measure),
+    # bracketed by barrier + synchronize, CUDA events on the engine's stream; repeated, and the MEDIAN region is reported
+    def timed_region(K):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        es = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K)]
+        barrier()
+        l0 = eng.launch_count()
+        ev0.record()
+        for k in range(K):
+            es[2 * k].record()
+            eng.sweep(n_or, n_hb)
+            es[2 * k + 1].record()
+            eng.pt_swap(out=acc)
+            if measure:
+                eng.measure(out=outs)
+        ev1.record()
+        barrier()
+        t = [ev0.elapsed_time(ev1), sum(es[2 * k].elapsed_time(es[2 * k + 1]) for k in range(K))]
+        if dist is not None:
+            tt = torch.tensor(t, device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            t = tt.tolist()
+        return t[0], t[1], eng.launch_count() - l0
+
+    first_ms, _, _ = timed_region(args.steps)                  # one untimed-in-the-report region sizes the repeat count
+    if args.repeats > 0:
+        n_rep = args.repeats
+    else:                                                      # at least 5 repeats and at least ~1 s of timed work in total
+        n_rep = int(min(50, max(5, np.ceil(1000.0 / max(first_ms, 1e-3)))))
+    if dist is not None:
+        tt = torch.tensor([n_rep], device="cuda"); dist.all_reduce(tt, op=dist.ReduceOp.MAX); n_rep = int(tt.item())
     sampler = ClockSampler(local) if rank == 0 else None
     if sampler:
         sampler.start()
-    launches0 = eng.launch_count()
-    fuse = not args.no_fuse_energy
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * args.steps + 2)]
-    ev_mid = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    ev[0].record()
-    for k in range(args.steps):
-        ev[2 + 2 * k].record()
-        if two_phase:                      # exactly the two launches hsg_sweep(n_or, n_hb) makes: E and m only in the last one
+    regions = [timed_region(args.steps) for _ in range(n_rep)]
+    clocks = sampler.stop() if sampler else None
+    totals = sorted(r[0] for r in regions)
+    total_ms = float(np.median(totals))
+    sweep_ms = float(np.median([r[1] for r in regions]))
+    launches = regions[0][2]
+
+    # ---- per-launch breakdown (roofline only): at L = 32 / 16 hsg_sweep(n_or, n_hb) is an over-relaxation launch followed by
+    # a heat-bath launch; a separate pass makes the same two launches through two calls so that each can be timed
+    or_ms = 0.0
+    if two_phase:
+        K2 = min(args.steps, 20)
+        fuse = not args.no_fuse_energy
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3 * K2)]
+        barrier()
+        for k in range(K2):
+            ev[3 * k].record()
             if fuse:
-                eng.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
+                eng.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)         # E and m only in the last launch, as in the single call
             eng.sweep(n_or, 0)
-            ev_mid[k].record()
+            ev[3 * k + 1].record()
             if fuse:
                 eng.set_option(hsg.HSG_OPT_FUSE_ENERGY, 1)
             eng.sweep(0, n_hb)
-        else:
-            eng.sweep(n_or, n_hb)
-        ev[3 + 2 * k].record()
-        eng.pt_swap(out=acc)
-        if measure:
-            eng.measure(out=outs)
-    ev[1].record()
-    barrier()
-    launches = eng.launch_count() - launches0
-    clocks = sampler.stop() if sampler else None
-    total_ms = ev[0].elapsed_time(ev[1])
-    sweep_ms = sum(ev[2 + 2 * k].elapsed_time(ev[3 + 2 * k]) for k in range(args.steps))
-    or_ms = sum(ev[2 + 2 * k].elapsed_time(ev_mid[k]) for k in range(args.steps)) if two_phase else 0.0
-    if dist is not None:
-        t = torch.tensor([total_ms, sweep_ms, or_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, sweep_ms, or_ms = t.tolist()
+            ev[3 * k + 2].record()
+            eng.pt_swap(out=acc)
+            if measure:
+                eng.measure(out=outs)
+        barrier()
+        or_k = float(np.median([ev[3 * k].elapsed_time(ev[3 * k + 1]) for k in range(K2)]))
+        hb_k = float(np.median([ev[3 * k + 1].elapsed_time(ev[3 * k + 2]) for k in range(K2)]))
+        if dist is not None:
+            tt = torch.tensor([or_k, hb_k], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            or_k, hb_k = tt.tolist()
+        or_ms, hb_ms = or_k * args.steps, hb_k * args.steps        # scaled to a region of args.steps steps, like sweep_ms
 
     # ---- end-to-end round through the C ABI from host buffers (rank-local; max over ranks)
     e2e = None
@@ -316,31 +352,38 @@ def main_ours(args, cfg, temps):
     bytes_per_update = 24.0 + 24.0 / (O * T)
     peak, peak_src = _peaks()
     sweeps_gbs = bytes_per_update * updates_step / (sweep_ms / args.steps * 1e-3) / 1e9      # all sweep launches of a step
+    step_gbs = bytes_per_update * updates_step / (total_ms / args.steps * 1e-3) / 1e9       # whole step (what `value` times)
     if two_phase:
-        # dominant kernel = the over-relaxation launch (n_or of the n_or + n_hb sweeps of a step)
+        # dominant kernel = the over-relaxation launch (n_or of the n_or + n_hb sweeps of a step), from the split pass
         per_launch_updates = n_or * R * N
         launch_ms = or_ms / args.steps
         kname, tkey = f"zmarch_kernel, over-relaxation launch ({n_or} sweeps)", "zmarch_or"
-        share = or_ms / total_ms
+        share = or_ms / (or_ms + hb_ms) * sweep_ms / total_ms
     else:
         per_launch_updates = updates_step / sweep_launches_per_call
         launch_ms = sweep_ms / args.steps / sweep_launches_per_call
         kname, tkey = f"sweep ({kernel}), {sweep_launches_per_call} launch(es) per step", kernel
         share = sweep_ms / total_ms
     achieved = bytes_per_update * per_launch_updates / (launch_ms * 1e-3) / 1e9
+    traffic, traffic_src = _traffic(args.workload, tkey)
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": _traffic(args.workload, tkey), "kernel": kname, "peak_source": peak_src,
+                "traffic": traffic, "traffic_source": traffic_src, "kernel": kname, "peak_source": peak_src,
                 "bytes_per_update": bytes_per_update, "launch_ms": launch_ms, "kernel_share_of_step": share,
+                # the metric is the OR+HB mix: the same fraction over ALL sweep launches of a step and over the whole step
+                "frac_all_sweeps": sweeps_gbs / peak, "frac_whole_step": step_gbs / peak,
                 "all_sweeps": {"achieved": sweeps_gbs, "frac": sweeps_gbs / peak, "ms": sweep_ms / args.steps,
                                "share_of_step": sweep_ms / total_ms,
-                               "heat_bath_launch_ms": (sweep_ms - or_ms) / args.steps if two_phase else None}}
+                               "heat_bath_launch_ms": hb_ms / args.steps if two_phase else None},
+                "whole_step": {"achieved": step_gbs, "frac": step_gbs / peak, "ms": total_ms / args.steps}}
 
     if args.cpu_steps > 0:
         ns_cpu, cores, text, _ = run_oracle(cfg, temps, args.cpu_steps, 1)
     else:
         ns_cpu, cores, text = None, 0, "skipped (--cpu-steps 0)"
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "ms_per_step": ms_step, "repeats": n_rep, "timed_region_s": total_ms * 1e-3, "timed_total_s": sum(totals) * 1e-3,
+            "value_min": totals[0] / args.steps * 1e6 / updates_step / world, "value_max": totals[-1] / args.steps * 1e6 / updates_step / world,
+            "spread": (totals[-1] - totals[0]) / total_ms, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": f"{args.workload}: L={L}, {D} samples x {O} replicas x {T} temperatures per GPU, "
                                    f"{n_or} OR + {n_hb} HB + PT{' + measure' if measure else ''} per step",
@@ -359,8 +402,9 @@ def main_ours(args, cfg, temps):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=100, help="steps per timed region (SURVEY 8(d): 20 warm-up + 100 timed steps, repeated)")
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--repeats", type=int, default=0, help="timed regions (each exactly --steps steps); the median is reported. 0 = at least 5 and at least ~1 s in total")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", choices=sorted(hsg_inputs.CONFIGS))
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "zmarch"])

@@ -18,7 +18,8 @@
  *   - Every call only ENQUEUES work on the CUDA stream given to hsg_create() (a cudaStream_t passed
  *     as void*; NULL = the legacy default stream) and returns without synchronising; outputs are valid
  *     once the caller has synchronised that stream.  The device current at hsg_create() must be
- *     current at every later call.
+ *     current at every later call (checked: HSG_ESTATE otherwise); contexts on different devices of one
+ *     process are independent.
  *   - Site index i = x + L*(y + L*z), x fastest.  N = L^3.
  *     J_dev[d][dir][i]: coupling of the bond from site i to site i+e_dir (dir 0,1,2 = x,y,z), periodic.
  *     H_dev[d][c][i]  : component c of the field at site i.
@@ -77,8 +78,10 @@ typedef struct {
   uint64_t sample_offset;/* global id of local sample 0: random streams are keyed by the global id
                             sample_offset+d, so a job sharded by sample over several GPUs
                             reproduces the single-GPU run */
-  uint32_t flags;        /* reserved, must be 0 */
+  uint32_t flags;        /* HSG_FLAG_* bits; 0 = the reference arithmetic of DESIGN.md §3 */
 } hsg_desc;
+/* Limits checked by hsg_query_bytes / hsg_create (HSG_EINVAL otherwise): L^3 < 2^31 (the site index is a 32-bit word
+ * of the random-stream counter) and (sample_offset + D) * O * T < 2^32 (so is the global system id). */
 
 /* Sizes of the two caller-owned device buffers for this descriptor. */
 int hsg_query_bytes(const hsg_desc* desc, size_t* state_bytes, size_t* scratch_bytes);
@@ -133,9 +136,45 @@ int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, doub
 
 /* Checkpoint: slot_of_temp_dev [D][O][T] int32 = configuration slot (0..T-1 within its (d,o) group, in
  * hsg_init order) that holds temperature t; counters_host = {heat-bath sweep counter, PT counter}.
- * hsg_get_state synchronises nothing: slot_of_temp_dev is written on the stream. */
+ * hsg_get_state synchronises nothing: slot_of_temp_dev is written on the stream.
+ * Restore order: hsg_set_state(permutation) FIRST, then hsg_set_spins — spins arrive by temperature index and are
+ * stored in the slot the permutation in force at that moment assigns; a later hsg_set_state re-labels the
+ * configurations without moving them. */
 int hsg_get_state(hsg_ctx* ctx, int32_t* slot_of_temp_dev, uint64_t counters_host[2]);
 int hsg_set_state(hsg_ctx* ctx, const int32_t* slot_of_temp_dev, const uint64_t counters_host[2]);
+
+/* Field-case observables (Eqs. 9-11): the susceptibility summands of Eq. (10) from four real replicas
+ * (1),(2),(3),(4) = replicas 0,1,2,3 of every sample, all at temperature index t, for k = 0 and
+ * k_min = (2 pi/L)(1,0,0):
+ *   chi_1(k) = sum_{i,j} sum_{mu,nu} s_i^{mu(1)} s_j^{nu(1)} s_i^{mu(2)} s_j^{nu(2)} e^{ik.(R_i-R_j)}
+ *   chi_2(k) = ...                   s_i^{mu(1)} s_j^{nu(1)} s_i^{mu(3)} s_j^{nu(4)} ...
+ *   chi_3(k) = ...                   s_i^{mu(1)} s_j^{nu(2)} s_i^{mu(3)} s_j^{nu(4)} ...
+ * chi_dev [D][T][2 (k = 0, k_min)][3 (chi_1, chi_2, chi_3)][2 (re, im)] fp64.  The thermal average of Eq. (10) is the
+ * caller's mean over measurements; Eq. (11): chi_SG(k) = (1/N) [chi_1 - 2 chi_2 + chi_3]_J.  Needs O >= 4
+ * (HSG_EUNSUPPORTED otherwise).  Evaluated as products of A_ab(k) = sum_i (s_i^(a).s_i^(b)) e^{ik x_i}. */
+int hsg_measure_field(hsg_ctx* ctx, double* chi_dev);
+
+/* Chiral sector: local chirality kappa_i^alpha = s_{i+alpha} . (s_i x s_{i-alpha}) (Eq. 12, alpha = x,y,z,
+ * periodic; formed in single precision in the operation order of DESIGN.md §3.8) and the chiral overlaps (Eq. 13)
+ *   qc0_dev [D][P][T][3]     q_c^alpha(0)     = (1/N) sum_i kappa_i^{alpha(a)} kappa_i^{alpha(b)}
+ *   qck_dev [D][P][T][3][2]  q_c^alpha(k_min) = (1/N) sum_i kappa_i^{alpha(a)} kappa_i^{alpha(b)} e^{+i k x_i}   (re, im)
+ * for replica pairs a<b at the same temperature (fp64 products and sums); either pointer may be NULL.
+ * chi_CG^alpha(k) = N <|q_c^alpha(k)|^2> (Eq. 14) and xi_c (Eq. 15, hsg_xi_second_moment) are the caller's averages. */
+int hsg_measure_chiral(hsg_ctx* ctx, double* qc0_dev, double* qck_dev);
+
+/* Second-moment correlation length, Eq. (8) (and Eq. 15): xi = sqrt(chi(0)/chi(k_min) - 1) / (2 sin(k_min/2)),
+ * |k_min| = 2 pi/L.  Host arithmetic on host values; HSG_EINVAL if chi_kmin <= 0 or the ratio is below 1. */
+int hsg_xi_second_moment(double chi_0, double chi_kmin, int32_t L, double* xi_host);
+
+/* Parallel-tempering diagnostics (PAPER.md:197 and Fig. 3), accumulated on the device by hsg_pt_swap once
+ * hsg_pt_diag_reset() has been called (which zeroes them and marks the configurations that start at an end point):
+ *   moved_dev      [D][O][T] int64, by temperature index: passes after which the copy that held T_t had left it
+ *   traversals_dev [D][O][T] int64, by configuration slot: arrivals at one end point of the ladder after the last touch
+ *                  of the other one; N_tunn ("a replica travels a closed loop between T_1 and T_{R_T}") = traversals / 2
+ *   p_diff_dev     [T] fp64: moved summed over (d,o) / (D O n_pass) — the quantity of Fig. 3
+ *   n_pass_host    passes counted since the reset.  Any pointer may be NULL. */
+int hsg_pt_diag_reset(hsg_ctx* ctx);
+int hsg_pt_diag_get(hsg_ctx* ctx, int64_t* moved_dev, int64_t* traversals_dev, double* p_diff_dev, uint64_t* n_pass_host);
 
 /* Tuning / test hooks (HSG_OPT_*).  Results never depend on them. */
 int hsg_set_option(hsg_ctx* ctx, int option, int value);

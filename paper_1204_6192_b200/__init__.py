@@ -27,6 +27,7 @@ SYMBOLS = (
     "hsg_query_bytes", "hsg_create", "hsg_destroy", "hsg_set_disorder", "hsg_init_spins", "hsg_set_spins",
     "hsg_get_spins", "hsg_sweep", "hsg_energy", "hsg_pt_swap", "hsg_measure", "hsg_get_state", "hsg_set_state",
     "hsg_set_option", "hsg_launch_count", "hsg_last_sweep_kernel", "hsg_last_error", "hsg_version", "hsg_selftest_arith",
+    "hsg_measure_field", "hsg_measure_chiral", "hsg_xi_second_moment", "hsg_pt_diag_reset", "hsg_pt_diag_get",
 )
 
 
@@ -71,6 +72,11 @@ def lib() -> C.CDLL:
         L.hsg_last_error.argtypes = [vp]; L.hsg_last_error.restype = C.c_char_p
         L.hsg_version.argtypes = []; L.hsg_version.restype = C.c_char_p
         L.hsg_selftest_arith.argtypes = [vp, C.c_uint64, C.c_uint64, vp]
+        L.hsg_measure_field.argtypes = [vp, vp]
+        L.hsg_measure_chiral.argtypes = [vp, vp, vp]
+        L.hsg_xi_second_moment.argtypes = [C.c_double, C.c_double, C.c_int32, C.POINTER(C.c_double)]
+        L.hsg_pt_diag_reset.argtypes = [vp]
+        L.hsg_pt_diag_get.argtypes = [vp, vp, vp, vp, C.POINTER(C.c_uint64)]
         _LIB = L
     return _LIB
 
@@ -89,6 +95,15 @@ def hsg_selftest_arith(n, seed=1):
     return tuple(int(x) for x in counts.cpu())
 
 
+def hsg_xi_second_moment(chi_0, chi_kmin, L) -> float:
+    """Eq. (8) / Eq. (15) of the paper through the C ABI (host arithmetic)."""
+    xi = C.c_double(0.0)
+    rc = lib().hsg_xi_second_moment(float(chi_0), float(chi_kmin), int(L), C.byref(xi))
+    if rc != HSG_OK:
+        raise HsgError(rc, "hsg_xi_second_moment: chi(0) >= chi(k_min) > 0 required")
+    return xi.value
+
+
 def hsg_query_bytes(L, n_samples, n_replicas, temps, seed=0, sample_offset=0):
     temps = np.ascontiguousarray(temps, dtype=np.float32)
     d = hsg_desc(int(L), int(n_samples), int(n_replicas), len(temps), temps.ctypes.data_as(C.POINTER(C.c_float)),
@@ -98,6 +113,18 @@ def hsg_query_bytes(L, n_samples, n_replicas, temps, seed=0, sample_offset=0):
     if rc != HSG_OK:
         raise HsgError(rc, "hsg_query_bytes: invalid descriptor")
     return a.value, b.value
+
+
+def _on_device(method):
+    """Run a method with the engine's device current (hsg.h: the device of hsg_create() must be current at every call),
+    so that engines on several devices can be driven from one process."""
+    import functools
+
+    @functools.wraps(method)
+    def wrapped(self, *a, **kw):
+        with self.torch.cuda.device(self.device):
+            return method(self, *a, **kw)
+    return wrapped
 
 
 class Hsg:
@@ -170,6 +197,7 @@ class Hsg:
     def set_option(self, option, value):
         self._ck(lib().hsg_set_option(self._h, int(option), int(value)))
 
+    @_on_device
     def set_disorder(self, J, H=None):
         t = self.torch
         Jd = self._dev(J, t.float32, (self.D, 3, self.L, self.L, self.L))
@@ -177,27 +205,33 @@ class Hsg:
         self._ck(lib().hsg_set_disorder(self._h, Jd.data_ptr(), None if Hd is None else Hd.data_ptr()))
         self._keep = (Jd, Hd)      # stay alive until the pack kernel has run; freed at the next call
 
+    @_on_device
     def init_spins(self):
         self._ck(lib().hsg_init_spins(self._h))
 
+    @_on_device
     def set_spins(self, S):
         Sd = self._dev(S, self.torch.float32, (self.D, self.O, self.T, 3, self.L, self.L, self.L))
         self._ck(lib().hsg_set_spins(self._h, Sd.data_ptr()))
         self._keep_s = Sd
 
+    @_on_device
     def get_spins(self, out=None):
         S = out if out is not None else self._new((self.D, self.O, self.T, 3, self.L, self.L, self.L), self.torch.float32)
         self._ck(lib().hsg_get_spins(self._h, S.data_ptr()))
         return S
 
+    @_on_device
     def sweep(self, n_or, n_hb):
         self._ck(lib().hsg_sweep(self._h, int(n_or), int(n_hb)))
 
+    @_on_device
     def energy(self, out=None):
         E = out if out is not None else self._new((self.D, self.O, self.T), self.torch.float64)
         self._ck(lib().hsg_energy(self._h, E.data_ptr()))
         return E
 
+    @_on_device
     def pt_swap(self, out=None, want_flags=True):
         acc = None
         if want_flags:
@@ -205,6 +239,7 @@ class Hsg:
         self._ck(lib().hsg_pt_swap(self._h, None if acc is None else acc.data_ptr()))
         return acc
 
+    @_on_device
     def measure(self, out=None):
         t = self.torch
         if out is None:
@@ -214,12 +249,43 @@ class Hsg:
         self._ck(lib().hsg_measure(self._h, *(None if x is None else x.data_ptr() for x in (E, M, q0, qk))))
         return E, M, q0, qk
 
+    @_on_device
+    def measure_field(self, out=None):
+        chi = out if out is not None else self._new((self.D, self.T, 2, 3, 2), self.torch.float64)
+        self._ck(lib().hsg_measure_field(self._h, chi.data_ptr()))
+        return chi
+
+    @_on_device
+    def measure_chiral(self, out=None):
+        t = self.torch
+        if out is None:
+            out = (self._new((self.D, self.P, self.T, 3), t.float64), self._new((self.D, self.P, self.T, 3, 2), t.float64))
+        qc0, qck = out
+        self._ck(lib().hsg_measure_chiral(self._h, *(None if x is None else x.data_ptr() for x in (qc0, qck))))
+        return qc0, qck
+
+    @_on_device
+    def pt_diag_reset(self):
+        self._ck(lib().hsg_pt_diag_reset(self._h))
+
+    @_on_device
+    def pt_diag_get(self):
+        """(moved[D][O][T], traversals[D][O][T], p_diff[T]) device tensors and the number of passes counted."""
+        t = self.torch
+        moved, trav = self._new((self.D, self.O, self.T), t.int64), self._new((self.D, self.O, self.T), t.int64)
+        p_diff = self._new((self.T,), t.float64)
+        n = C.c_uint64(0)
+        self._ck(lib().hsg_pt_diag_get(self._h, moved.data_ptr(), trav.data_ptr(), p_diff.data_ptr(), C.byref(n)))
+        return moved, trav, p_diff, int(n.value)
+
+    @_on_device
     def get_state(self):
         perm = self._new((self.D, self.O, self.T), self.torch.int32)
         cnt = (C.c_uint64 * 2)()
         self._ck(lib().hsg_get_state(self._h, perm.data_ptr(), cnt))
         return perm, (int(cnt[0]), int(cnt[1]))
 
+    @_on_device
     def set_state(self, perm=None, counters=None):
         p = self._dev(perm, self.torch.int32, (self.D, self.O, self.T))
         cnt = None if counters is None else (C.c_uint64 * 2)(int(counters[0]), int(counters[1]))

@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 
 #include "hsg_kernels.cuh"
+#include "hsg_observables.cuh"
 #include "hsg_zmarch_launch.h"
 
 using namespace hsg;
@@ -23,7 +24,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 // carve-up of the caller's two buffers (offsets in bytes)
 struct StateLayout {
-  size_t spins, jh, slot_of_temp, temp_of_slot, beta, cs_table, e_slot, m_slot, total;
+  size_t spins, jh, slot_of_temp, temp_of_slot, beta, cs_table, e_slot, m_slot, diag_moved, diag_trav, diag_last, total;
 };
 struct ScratchLayout {
   size_t e_partial, q_partial, total;
@@ -40,6 +41,9 @@ StateLayout state_layout(const Geom& g) {
   s.cs_table = o;     o = align_up(o + sizeof(double) * 2 * g.L);
   s.e_slot = o;       o = align_up(o + sizeof(double) * g.R);
   s.m_slot = o;       o = align_up(o + sizeof(double) * 3 * g.R);
+  s.diag_moved = o;   o = align_up(o + sizeof(long long) * g.R);
+  s.diag_trav = o;    o = align_up(o + sizeof(long long) * g.R);
+  s.diag_last = o;    o = align_up(o + sizeof(int32_t) * g.R);
   s.total = o;
   return s;
 }
@@ -48,7 +52,8 @@ ScratchLayout scratch_layout(const Geom& g) {
   const size_t P = (size_t)g.O * (g.O - 1) / 2;
   size_t o = 0;
   s.e_partial = o; o = align_up(o + sizeof(double) * 4 * (size_t)g.R * g.L);
-  s.q_partial = o; o = align_up(o + sizeof(double) * 27 * (size_t)g.D * P * g.T * g.L);
+  // 27 doubles per (d, pair, t, chunk) for the overlaps; also used for the chiral (9) and field-case (12 per (d, t, chunk)) partials
+  s.q_partial = o; o = align_up(o + sizeof(double) * 27 * (size_t)g.D * (P > 0 ? P : 1) * g.T * g.L);
   s.total = o;
   return s;
 }
@@ -64,6 +69,8 @@ int check_desc(const hsg_desc* d) {
   const double n = (double)d->L * d->L * d->L;
   if (n > 2147483647.0) return HSG_EINVAL;                                   // site index is the 32-bit Philox word c0
   if ((double)d->n_samples * d->n_replicas * d->n_temps > 1.0e9) return HSG_EINVAL;
+  // the global system id ((sample_offset + d) * O + o) * T + t is a 32-bit word of the random-stream counter
+  if (((double)d->sample_offset + (double)d->n_samples) * d->n_replicas * d->n_temps >= 4294967296.0) return HSG_EINVAL;
   return HSG_OK;
 }
 
@@ -89,6 +96,8 @@ struct hsg_ctx {
   // device pointers into the caller's buffers
   float* spins; float* jh; int32_t* slot_of_temp; int32_t* temp_of_slot; float* beta; double* cs_table;
   double* e_slot; double* m_slot; double* e_partial; double* q_partial;
+  long long* diag_moved; long long* diag_trav; int32_t* diag_last;     // parallel-tempering diagnostics (hsg_pt_diag_*)
+  bool diag_on; unsigned long long diag_passes;
   unsigned long long k_hb, k_pt;
   bool have_disorder, have_spins;
   bool energy_valid;            // e_slot / m_slot hold the reduction of the current spins
@@ -101,6 +110,11 @@ struct hsg_ctx {
   std::string err;
 };
 
+// every call on a context: non-null, and the device it was created on is current (hsg.h)
+#define HSG_ENTER(ctx) do { if (!(ctx)) return HSG_EINVAL; int dev_ = -1; \
+  if (cudaGetDevice(&dev_) != cudaSuccess || dev_ != (ctx)->device) { \
+    (ctx)->err = "the CUDA device current at hsg_create() (" + std::to_string((ctx)->device) + ") is not current (" + std::to_string(dev_) + ")"; \
+    return HSG_ESTATE; } } while (0)
 #define HSG_FAIL(ctx, code, msg) do { (ctx)->err = (msg); return (code); } while (0)
 #define HSG_CUDA(ctx, expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { \
   (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(e_); return HSG_ECUDA; } } while (0)
@@ -145,6 +159,8 @@ int hsg_create(const hsg_desc* desc, void* dev_state, size_t state_bytes, void* 
   c->beta = (float*)(s + sl.beta); c->cs_table = (double*)(s + sl.cs_table);
   c->e_slot = (double*)(s + sl.e_slot); c->m_slot = (double*)(s + sl.m_slot);
   c->e_partial = (double*)(w + cl.e_partial); c->q_partial = (double*)(w + cl.q_partial);
+  c->diag_moved = (long long*)(s + sl.diag_moved); c->diag_trav = (long long*)(s + sl.diag_trav); c->diag_last = (int32_t*)(s + sl.diag_last);
+  c->diag_on = false; c->diag_passes = 0;
   c->k_hb = 0; c->k_pt = 0; c->have_disorder = false; c->have_spins = false; c->energy_valid = false;
   c->sweep_kernel_opt = HSG_KERNEL_AUTO; c->fuse_energy = true; c->last_kernel = "none"; c->launches = 0;
 
@@ -194,7 +210,7 @@ int hsg_set_option(hsg_ctx* ctx, int option, int value) {
 }
 
 int hsg_set_disorder(hsg_ctx* ctx, const float* J_dev, const float* H_dev) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (!J_dev) HSG_FAIL(ctx, HSG_EINVAL, "J_dev is null");
   pack_disorder_kernel<<<blocks_for((long long)ctx->g.D * ctx->g.N), kThreads, 0, ctx->stream>>>(ctx->g, J_dev, H_dev, ctx->jh);
   HSG_LAUNCHED(ctx);
@@ -204,7 +220,7 @@ int hsg_set_disorder(hsg_ctx* ctx, const float* J_dev, const float* H_dev) {
 }
 
 int hsg_init_spins(hsg_ctx* ctx) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   init_spins_kernel<<<blocks_for((long long)ctx->g.R * ctx->g.N), kThreads, 0, ctx->stream>>>(ctx->g, ctx->key, ctx->temp_of_slot, ctx->spins);
   HSG_LAUNCHED(ctx);
   ctx->have_spins = true;
@@ -213,7 +229,7 @@ int hsg_init_spins(hsg_ctx* ctx) {
 }
 
 int hsg_set_spins(hsg_ctx* ctx, const float* S_dev) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (!S_dev) HSG_FAIL(ctx, HSG_EINVAL, "S_dev is null");
   convert_spins_kernel<true><<<blocks_for((long long)ctx->g.R * ctx->g.N), kThreads, 0, ctx->stream>>>(
       ctx->g, ctx->slot_of_temp, ctx->spins, const_cast<float*>(S_dev));
@@ -224,7 +240,7 @@ int hsg_set_spins(hsg_ctx* ctx, const float* S_dev) {
 }
 
 int hsg_get_spins(hsg_ctx* ctx, float* S_dev) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (!S_dev) HSG_FAIL(ctx, HSG_EINVAL, "S_dev is null");
   if (!ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "spins not set");
   convert_spins_kernel<false><<<blocks_for((long long)ctx->g.R * ctx->g.N), kThreads, 0, ctx->stream>>>(
@@ -250,7 +266,7 @@ static int launch_generic_sweep(hsg_ctx* ctx, bool hb) {
 }
 
 int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (n_or < 0 || n_hb < 0) HSG_FAIL(ctx, HSG_EINVAL, "negative sweep count");
   if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_sweep before disorder and spins were set");
   if (n_or + n_hb == 0) return HSG_OK;
@@ -291,6 +307,15 @@ static int reduce_zb(const Geom& g, int V) {
 }
 static int vec_width(const Geom& g) { return (g.Lh % 4 == 0) ? 4 : (g.Lh % 2 == 0) ? 2 : 1; }
 
+// a block takes a chunk of planes of one (sample[, pair], temperature): whole lattices up to L = 32, 16 planes beyond
+static void reduction_shape(const Geom& g, int V, int* ZB, int* n_chunks, int* nt) {
+  *ZB = g.L > 32 ? 16 : g.L;
+  *n_chunks = (g.L + *ZB - 1) / *ZB;
+  int n = 32;
+  while (n < kThreads && ((long long)*ZB * g.L * (g.Lh / V) >= 8LL * n || n < 2 * (g.Lh / V))) n *= 2;
+  *nt = n;
+}
+
 static int enqueue_energy_mag(hsg_ctx* ctx) {
   const Geom& g = ctx->g;
   if (ctx->energy_valid) return HSG_OK;          // spins unchanged since the last reduction
@@ -307,7 +332,7 @@ static int enqueue_energy_mag(hsg_ctx* ctx) {
 }
 
 int hsg_energy(hsg_ctx* ctx, double* E_dev) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (!E_dev) HSG_FAIL(ctx, HSG_EINVAL, "E_dev is null");
   if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_energy before disorder and spins were set");
   const int rc = enqueue_energy_mag(ctx);
@@ -318,19 +343,21 @@ int hsg_energy(hsg_ctx* ctx, double* E_dev) {
 }
 
 int hsg_pt_swap(hsg_ctx* ctx, int32_t* accepted_dev) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_pt_swap before disorder and spins were set");
   const int rc = enqueue_energy_mag(ctx);
   if (rc != HSG_OK) return rc;
   pt_swap_kernel<<<blocks_for((long long)ctx->g.D * ctx->g.O), kThreads, 0, ctx->stream>>>(
-      ctx->g, ctx->key, ctx->k_pt, ctx->beta, ctx->e_slot, ctx->slot_of_temp, ctx->temp_of_slot, accepted_dev);
+      ctx->g, ctx->key, ctx->k_pt, ctx->beta, ctx->e_slot, ctx->slot_of_temp, ctx->temp_of_slot, accepted_dev,
+      ctx->diag_on ? PtDiag{ctx->diag_moved, ctx->diag_trav, ctx->diag_last} : PtDiag{nullptr, nullptr, nullptr});
   HSG_LAUNCHED(ctx);
   ++ctx->k_pt;
+  if (ctx->diag_on) ++ctx->diag_passes;
   return HSG_OK;
 }
 
 int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, double* qk_dev) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (!ctx->have_disorder || !ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_measure before disorder and spins were set");
   const Geom& g = ctx->g;
   if (E_dev || M_dev) {
@@ -342,12 +369,10 @@ int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, doub
   const int P = g.O * (g.O - 1) / 2;
   if ((q0_dev || qk_dev) && P > 0) {
     const long long n_sys = (long long)g.D * P * g.T;
-    // a block takes whole systems (chunks of 16 planes at L = 64) with enough (y,z) rows per thread to amortise the
-    // per-pass phase fold: about 8 rows per thread and x-parity, at least one warp, at most kThreads
-    const int V = vec_width(g), ZB = g.L > 32 ? 16 : g.L, n_chunks = (g.L + ZB - 1) / ZB;
+    const int V = vec_width(g);
+    int ZB, n_chunks, nt;
+    reduction_shape(g, V, &ZB, &n_chunks, &nt);
     const unsigned nb = (unsigned)(n_sys * n_chunks);
-    int nt = 32;
-    while (nt < kThreads && ((long long)ZB * g.L * (g.Lh / V) >= 8LL * nt || nt < 2 * (g.Lh / V))) nt *= 2;
     if (V == 4) overlap_kernel<4><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
     else if (V == 2) overlap_kernel<2><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
     else overlap_kernel<1><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
@@ -355,6 +380,77 @@ int hsg_measure(hsg_ctx* ctx, double* E_dev, double* M_dev, double* q0_dev, doub
     finalize_overlap_kernel<<<blocks_for(n_sys * 9), kThreads, 0, ctx->stream>>>(g, (int)n_sys, n_chunks, ctx->q_partial, q0_dev, qk_dev);
     HSG_LAUNCHED(ctx);
   }
+  return HSG_OK;
+}
+
+// ------------------------------------------------------------------ field case, chirality, PT diagnostics
+int hsg_measure_field(hsg_ctx* ctx, double* chi_dev) {
+  HSG_ENTER(ctx);
+  if (!chi_dev) HSG_FAIL(ctx, HSG_EINVAL, "chi_dev is null");
+  if (!ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_measure_field before spins were set");
+  const Geom& g = ctx->g;
+  if (g.O < 4) HSG_FAIL(ctx, HSG_EUNSUPPORTED, "hsg_measure_field needs four replicas (PAPER.md:77)");
+  const int V = vec_width(g);
+  int ZB, n_chunks, nt;
+  reduction_shape(g, V, &ZB, &n_chunks, &nt);
+  const int n_dt = g.D * g.T;
+  const unsigned nb = (unsigned)((long long)n_dt * n_chunks);
+  if (V == 4) field_trace_kernel<4><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+  else if (V == 2) field_trace_kernel<2><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+  else field_trace_kernel<1><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+  HSG_LAUNCHED(ctx);
+  finalize_field_kernel<<<blocks_for(n_dt), kThreads, 0, ctx->stream>>>(n_dt, n_chunks, ctx->q_partial, chi_dev);
+  HSG_LAUNCHED(ctx);
+  return HSG_OK;
+}
+
+int hsg_measure_chiral(hsg_ctx* ctx, double* qc0_dev, double* qck_dev) {
+  HSG_ENTER(ctx);
+  if (!ctx->have_spins) HSG_FAIL(ctx, HSG_ESTATE, "hsg_measure_chiral before spins were set");
+  const Geom& g = ctx->g;
+  const int P = g.O * (g.O - 1) / 2;
+  if (P == 0 || (!qc0_dev && !qck_dev)) return HSG_OK;
+  const int V = vec_width(g);
+  int ZB, n_chunks, nt;
+  reduction_shape(g, V, &ZB, &n_chunks, &nt);
+  const long long n_sys = (long long)g.D * P * g.T;
+  const unsigned nb = (unsigned)(n_sys * n_chunks);
+  if (V == 4) chiral_kernel<4><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+  else if (V == 2) chiral_kernel<2><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+  else chiral_kernel<1><<<nb, nt, 0, ctx->stream>>>(g, ZB, ctx->spins, ctx->slot_of_temp, ctx->cs_table, ctx->q_partial);
+  HSG_LAUNCHED(ctx);
+  finalize_chiral_kernel<<<blocks_for(n_sys * 3), kThreads, 0, ctx->stream>>>(g, (int)n_sys, n_chunks, ctx->q_partial, qc0_dev, qck_dev);
+  HSG_LAUNCHED(ctx);
+  return HSG_OK;
+}
+
+int hsg_xi_second_moment(double chi_0, double chi_kmin, int32_t L, double* xi_host) {
+  if (!xi_host || L < 2 || !(chi_kmin > 0.0) || !(chi_0 >= chi_kmin)) return HSG_EINVAL;
+  const double kmin = 6.283185307179586476925286766559 / (double)L;
+  *xi_host = std::sqrt(chi_0 / chi_kmin - 1.0) / (2.0 * std::sin(0.5 * kmin));
+  return HSG_OK;
+}
+
+int hsg_pt_diag_reset(hsg_ctx* ctx) {
+  HSG_ENTER(ctx);
+  pt_diag_reset_kernel<<<blocks_for((long long)ctx->g.D * ctx->g.O), kThreads, 0, ctx->stream>>>(
+      ctx->g, ctx->slot_of_temp, ctx->diag_moved, ctx->diag_trav, ctx->diag_last);
+  HSG_LAUNCHED(ctx);
+  ctx->diag_on = true; ctx->diag_passes = 0;
+  return HSG_OK;
+}
+
+int hsg_pt_diag_get(hsg_ctx* ctx, int64_t* moved_dev, int64_t* traversals_dev, double* p_diff_dev, uint64_t* n_pass_host) {
+  HSG_ENTER(ctx);
+  if (!ctx->diag_on) HSG_FAIL(ctx, HSG_ESTATE, "hsg_pt_diag_get before hsg_pt_diag_reset");
+  const size_t nb = sizeof(long long) * ctx->g.R;
+  if (moved_dev) HSG_CUDA(ctx, cudaMemcpyAsync(moved_dev, ctx->diag_moved, nb, cudaMemcpyDeviceToDevice, ctx->stream));
+  if (traversals_dev) HSG_CUDA(ctx, cudaMemcpyAsync(traversals_dev, ctx->diag_trav, nb, cudaMemcpyDeviceToDevice, ctx->stream));
+  if (p_diff_dev) {
+    pt_diag_pdiff_kernel<<<blocks_for(ctx->g.T), kThreads, 0, ctx->stream>>>(ctx->g, ctx->diag_passes, ctx->diag_moved, p_diff_dev);
+    HSG_LAUNCHED(ctx);
+  }
+  if (n_pass_host) *n_pass_host = ctx->diag_passes;
   return HSG_OK;
 }
 
@@ -370,7 +466,7 @@ int hsg_selftest_arith(void* cuda_stream, uint64_t seed, uint64_t n, unsigned lo
 
 // ------------------------------------------------------------------ checkpoint
 int hsg_get_state(hsg_ctx* ctx, int32_t* slot_of_temp_dev, uint64_t counters_host[2]) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (slot_of_temp_dev)
     HSG_CUDA(ctx, cudaMemcpyAsync(slot_of_temp_dev, ctx->slot_of_temp, sizeof(int32_t) * ctx->g.R, cudaMemcpyDeviceToDevice, ctx->stream));
   if (counters_host) { counters_host[0] = ctx->k_hb; counters_host[1] = ctx->k_pt; }
@@ -378,7 +474,7 @@ int hsg_get_state(hsg_ctx* ctx, int32_t* slot_of_temp_dev, uint64_t counters_hos
 }
 
 int hsg_set_state(hsg_ctx* ctx, const int32_t* slot_of_temp_dev, const uint64_t counters_host[2]) {
-  if (!ctx) return HSG_EINVAL;
+  HSG_ENTER(ctx);
   if (slot_of_temp_dev) {
     // NOTE: the caller must pass a valid permutation per (sample, replica); spins stay in their slots.
     set_perm_kernel<<<blocks_for(ctx->g.R), kThreads, 0, ctx->stream>>>(ctx->g, slot_of_temp_dev, ctx->slot_of_temp, ctx->temp_of_slot);

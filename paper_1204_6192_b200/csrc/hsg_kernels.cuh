@@ -327,16 +327,31 @@ __global__ void gather_by_temp_kernel(Geom g, int nv, const int32_t* __restrict_
 }
 
 // ------------------------------------------------------------------ parallel tempering, Eq. (4)
+// Diagnostics of PAPER.md:197 / Fig. 3 (hsg_pt_diag_*): a configuration that arrives at one end point of the ladder after it
+// last touched the OTHER end point has made one traversal (a closed loop T_1 -> T_{R_T} -> T_1 = two traversals).  Cold end first.
+__device__ __forceinline__ void pt_diag_touch(int T, const int32_t* slot_of_temp, long long* trav, int32_t* last_end) {
+#pragma unroll
+  for (int e = 0; e < 2; ++e) {
+    const int s = slot_of_temp[e == 0 ? 0 : T - 1];
+    const int32_t tag = e == 0 ? 1 : -1;
+    if (last_end[s] == -tag) ++trav[s];
+    last_end[s] = tag;
+  }
+}
+
+struct PtDiag { long long* moved; long long* trav; int32_t* last_end; };   // all null: diagnostics off
+
 // One thread per (sample, replica) walks the ladder from the lowest temperature.
 __global__ void pt_swap_kernel(Geom g, PhiloxKey key, unsigned long long k_pt, const float* __restrict__ beta,
                                const double* __restrict__ e_slot, int32_t* slot_of_temp, int32_t* temp_of_slot,
-                               int32_t* __restrict__ accepted) {
+                               int32_t* __restrict__ accepted, PtDiag diag) {
   const int grp = blockIdx.x * kThreads + threadIdx.x;
   if (grp >= g.D * g.O) return;
   const int base = grp * g.T;
   const uint32_t c2 = (uint32_t)(g.sample_offset * g.O + (unsigned long long)grp);
   const uint32_t c1 = (uint32_t)(k_pt & 0xFFFFFFFFull), c3 = counter_hi(k_pt, DOMAIN_PT);
   int sa = slot_of_temp[base];
+  int before = sa;                           // the slot that held temperature t before this pass (diagnostics)
   double Ea = e_slot[base + sa];
   for (int t = 0; t + 1 < g.T; ++t) {
     const int sb = slot_of_temp[base + t + 1];
@@ -345,11 +360,20 @@ __global__ void pt_swap_kernel(Geom g, PhiloxKey key, unsigned long long k_pt, c
     uint32_t w0, w1, w2, w3;
     philox4x32_10((uint32_t)t, c1, c2, c3, key.k0, key.k1, w0, w1, w2, w3);
     const bool acc = (x >= 0.0) || (log(u01_f64(w0)) < x);
+    const int fin = acc ? sb : sa;           // the slot that holds temperature t after this pass
     if (acc) {   // the configuration that held t now holds t+1 and is compared with t+2 next
       slot_of_temp[base + t] = sb; temp_of_slot[base + sb] = t;
       slot_of_temp[base + t + 1] = sa; temp_of_slot[base + sa] = t + 1;
     } else { sa = sb; Ea = Eb; }
     if (accepted) accepted[grp * (g.T - 1) + t] = acc ? 1 : 0;
+    if (diag.moved) {                        // temperature t is final now: p_diff counts the passes after which its copy has left
+      if (fin != before) ++diag.moved[base + t];
+      before = sb;                           // sb was read before this step could change position t+1
+    }
+  }
+  if (diag.moved) {
+    if (sa != before) ++diag.moved[base + g.T - 1];
+    pt_diag_touch(g.T, slot_of_temp + base, diag.trav + base, diag.last_end + base);
   }
 }
 
@@ -376,48 +400,48 @@ __global__ void __launch_bounds__(kThreads, 2) overlap_kernel(Geom g, int ZB, co
   const float* A = spins + (long long)sa * 3 * g.N;
   const float* B = spins + (long long)sb * 3 * g.N;
   const int z0 = chunk * ZB, nz = min(ZB, L - z0);
-  const int RT = (int)blockDim.x / (2 * qpr);     // row lanes per x-parity
-  const int q = (int)threadIdx.x % qpr, par = ((int)threadIdx.x / qpr) & 1, r = (int)threadIdx.x / (2 * qpr), j0 = q * V;
+  const int RT = max(1, (int)blockDim.x / (2 * qpr));     // row lanes per x-parity
   double acc[27];
 #pragma unroll
   for (int k = 0; k < 27; ++k) acc[k] = 0.0;
-  if (r < RT) {
-    {
-      double s9[V][9];
+  // one item = (group of V compact sites, x-parity, row lane); rows wider than the block (2*qpr > blockDim.x: odd Lh > 128,
+  // L > 1024) take their items in several passes
+  for (int item = threadIdx.x; item < 2 * qpr * RT; item += blockDim.x) {
+    const int q = item % qpr, par = (item / qpr) & 1, r = item / (2 * qpr), j0 = q * V;
+    double s9[V][9];
 #pragma unroll
-      for (int e = 0; e < V; ++e)
+    for (int e = 0; e < V; ++e)
 #pragma unroll
-        for (int k = 0; k < 9; ++k) s9[e][k] = 0.0;
-      for (int m = r; m < nz * L; m += RT) {
-        const int y = m % L, z = z0 + m / L;
-        const int c = (par + y + z) & 1;    // the colour whose sites of row (y,z) sit at x = 2j + par
-        Vec<V> av[3], bv[3];
+      for (int k = 0; k < 9; ++k) s9[e][k] = 0.0;
+    for (int m = r; m < nz * L; m += RT) {
+      const int y = m % L, z = z0 + m / L;
+      const int c = (par + y + z) & 1;    // the colour whose sites of row (y,z) sit at x = 2j + par
+      Vec<V> av[3], bv[3];
 #pragma unroll
-        for (int mu = 0; mu < 3; ++mu) {
-          av[mu] = ldv<V>(A + spin_index(g, z, c, mu, y, j0));
-          bv[mu] = ldv<V>(B + spin_index(g, z, c, mu, y, j0));
-        }
-#pragma unroll
-        for (int e = 0; e < V; ++e) {
-          double ad[3], bd[3];
-#pragma unroll
-          for (int mu = 0; mu < 3; ++mu) { ad[mu] = (double)av[mu].v[e]; bd[mu] = (double)bv[mu].v[e]; }
-#pragma unroll
-          for (int mu = 0; mu < 3; ++mu)
-#pragma unroll
-            for (int nu = 0; nu < 3; ++nu) s9[e][mu * 3 + nu] = fma(ad[mu], bd[nu], s9[e][mu * 3 + nu]);
-        }
+      for (int mu = 0; mu < 3; ++mu) {
+        av[mu] = ldv<V>(A + spin_index(g, z, c, mu, y, j0));
+        bv[mu] = ldv<V>(B + spin_index(g, z, c, mu, y, j0));
       }
 #pragma unroll
       for (int e = 0; e < V; ++e) {
-        const int x = 2 * (j0 + e) + par;
-        const double co = cs_table[2 * x], si = cs_table[2 * x + 1];
+        double ad[3], bd[3];
 #pragma unroll
-        for (int k = 0; k < 9; ++k) {
-          acc[k] += s9[e][k];
-          acc[9 + k] = fma(s9[e][k], co, acc[9 + k]);
-          acc[18 + k] = fma(s9[e][k], si, acc[18 + k]);
-        }
+        for (int mu = 0; mu < 3; ++mu) { ad[mu] = (double)av[mu].v[e]; bd[mu] = (double)bv[mu].v[e]; }
+#pragma unroll
+        for (int mu = 0; mu < 3; ++mu)
+#pragma unroll
+          for (int nu = 0; nu < 3; ++nu) s9[e][mu * 3 + nu] = fma(ad[mu], bd[nu], s9[e][mu * 3 + nu]);
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+      const int x = 2 * (j0 + e) + par;
+      const double co = cs_table[2 * x], si = cs_table[2 * x + 1];
+#pragma unroll
+      for (int k = 0; k < 9; ++k) {
+        acc[k] += s9[e][k];
+        acc[9 + k] = fma(s9[e][k], co, acc[9 + k]);
+        acc[18 + k] = fma(s9[e][k], si, acc[18 + k]);
       }
     }
   }
