@@ -7,6 +7,7 @@ is newer than it.
 from __future__ import annotations
 
 import os
+import re
 import shutil
 import subprocess
 from pathlib import Path
@@ -33,7 +34,7 @@ def _nvcc() -> str:
 
 
 def sources():
-    return sorted(CSRC.glob("*.cu")) + sorted(CSRC.glob("*.cuh")) + [HEADER]
+    return sorted(CSRC.glob("*.cu")) + sorted(CSRC.glob("*.cuh")) + sorted(CSRC.glob("*.h")) + [HEADER]
 
 
 def stale() -> bool:
@@ -43,33 +44,53 @@ def stale() -> bool:
     return any(p.stat().st_mtime > t for p in sources())
 
 
+def _deps(unit: Path) -> set:
+    """The files a translation unit includes (quoted includes, transitively)."""
+    seen, todo = set(), [unit]
+    while todo:
+        f = todo.pop()
+        if f in seen or not f.exists():
+            continue
+        seen.add(f)
+        for m in re.finditer(r'#include\s+"([^"]+)"', f.read_text()):
+            todo.append((f.parent / m.group(1)).resolve())
+    return seen
+
+
 def build(force: bool = False, verbose: bool = False) -> Path:
-    """Compile every translation unit under csrc/ (in parallel) and link lib/libhsg.so; returns its path."""
+    """Compile the translation units under csrc/ whose sources changed (in parallel; objects are kept under lib/obj/) and
+    link lib/libhsg.so; returns its path.  Fails loudly: there is no CPU fallback."""
     if not force and not stale():
         return LIB
-    LIB.parent.mkdir(parents=True, exist_ok=True)
-    objdir = LIB.parent / f"obj.tmp{os.getpid()}"
+    objdir = LIB.parent / "obj"
     objdir.mkdir(parents=True, exist_ok=True)
     nvcc = _nvcc()
     units = sorted(CSRC.glob("*.cu"))
-    cmds = [[nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", str(u), "-o", str(objdir / (u.stem + ".o"))] for u in units]
-    try:
-        procs = [subprocess.Popen(c, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for c in cmds]
-        outs = [p.communicate()[0] for p in procs]
-        for c, p, o in zip(cmds, procs, outs):
-            if p.returncode != 0:
-                raise RuntimeError("nvcc failed:\n" + " ".join(c) + "\n" + o)
-            if verbose:
-                print(o)
-        tmp = LIB.with_name(f"libhsg.tmp{os.getpid()}.so")
-        link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC",
-                *[str(objdir / (u.stem + ".o")) for u in units], "-o", str(tmp)]
-        res = subprocess.run(link, capture_output=True, text=True)
-        if res.returncode != 0:
-            raise RuntimeError("link failed:\n" + " ".join(link) + "\n" + res.stdout + res.stderr)
-        os.replace(tmp, LIB)
-    finally:
-        shutil.rmtree(objdir, ignore_errors=True)
+    flag_tag = " ".join(NVCC_FLAGS)
+    tag_file = objdir / "flags.txt"
+    if not tag_file.exists() or tag_file.read_text() != flag_tag:
+        force = True
+    todo = []
+    for u in units:
+        o = objdir / (u.stem + ".o")
+        if force or not o.exists() or any(d.stat().st_mtime > o.stat().st_mtime for d in _deps(u)):
+            todo.append((u, o))
+    cmds = [[nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", str(u), "-o", str(o)] for u, o in todo]
+    procs = [subprocess.Popen(c, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for c in cmds]
+    outs = [p.communicate()[0] for p in procs]
+    for c, p, o in zip(cmds, procs, outs):
+        if p.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + " ".join(c) + "\n" + o)
+        if verbose:
+            print(o)
+    tag_file.write_text(flag_tag)
+    tmp = LIB.with_name(f"libhsg.tmp{os.getpid()}.so")
+    link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC",
+            *[str(objdir / (u.stem + ".o")) for u in units], "-o", str(tmp)]
+    res = subprocess.run(link, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("link failed:\n" + " ".join(link) + "\n" + res.stdout + res.stderr)
+    os.replace(tmp, LIB)
     return LIB
 
 

@@ -500,6 +500,14 @@ __global__ void selftest_arith_kernel(PhiloxKey key, unsigned long long n, unsig
     const float b2 = __uint_as_float((w1 & 0x007FFFFFu) | (127u << 23)) + (float)(w3 & 1u);
     const float a2 = __uint_as_float((w3 & 0x807FFFFFu) | ((120u + (w3 >> 28)) << 23));
     if (__float_as_uint(div_rn(a2, b2)) != __float_as_uint(__fdiv_rn(a2, b2))) ++bad_div;
+    // the reciprocals +-1/b (the move uses them for 1/|h| and -1/(sigma + n_z)), and the packed instantiation of all three
+    if (__float_as_uint(rcp_rn<float, false>(x)) != __float_as_uint(__fdiv_rn(1.0f, x))) ++bad_div;
+    if (__float_as_uint(rcp_rn<float, true>(b2)) != __float_as_uint(__fdiv_rn(-1.0f, b2))) ++bad_div;
+    const F2 qp = div_rn(make_f2(a, a2), make_f2(b, b2));
+    if (fabsf(q2) >= 1.2e-38f && fabsf(q2) <= 3.0e38f && __float_as_uint(f2_lo(qp)) != __float_as_uint(q2)) ++bad_div;
+    if (__float_as_uint(f2_hi(qp)) != __float_as_uint(__fdiv_rn(a2, b2))) ++bad_div;
+    const F2 rp = sqrt_rn(make_f2(x, b2));
+    if (__float_as_uint(f2_lo(rp)) != __float_as_uint(__fsqrt_rn(x)) || __float_as_uint(f2_hi(rp)) != __float_as_uint(__fsqrt_rn(b2))) ++bad_sqrt;
   }
   if (bad_div) atomicAdd(counts, (unsigned long long)bad_div);
   if (bad_sqrt) atomicAdd(counts + 1, (unsigned long long)bad_sqrt);

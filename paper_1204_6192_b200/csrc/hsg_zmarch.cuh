@@ -102,41 +102,34 @@ __device__ __forceinline__ void st_cluster_f64(uint32_t addr, double v) {
   asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
 }
 
-// ---------------------------------------------------------------- V-wide vector access (V = 2 or 4 floats)
-template <int V> struct VT;
-template <> struct VT<2> { using type = float2; };
-template <> struct VT<4> { using type = float4; };
+// ---------------------------------------------------------------- V-wide vector access: V = 2 or 4 floats = V/2 packed pairs
+// (hsg_math.cuh: F2 = two binary32 lanes in an aligned register pair; lane e&1 of pair e>>1 is compact site j0 + e)
 
 // shared memory by 32-bit shared-window byte address (keeps all address arithmetic 32-bit)
-template <int V> __device__ __forceinline__ void lds(float (&r)[V], uint32_t a);
-template <> __device__ __forceinline__ void lds<2>(float (&r)[2], uint32_t a) {
-  asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(r[0]), "=f"(r[1]) : "r"(a) : "memory");
+template <int V> __device__ __forceinline__ void lds(F2 (&r)[V / 2], uint32_t a);
+template <> __device__ __forceinline__ void lds<2>(F2 (&r)[1], uint32_t a) {
+  asm volatile("ld.shared.b64 %0, [%1];" : "=l"(r[0].v) : "r"(a) : "memory");
 }
-template <> __device__ __forceinline__ void lds<4>(float (&r)[4], uint32_t a) {
-  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(r[0]), "=f"(r[1]), "=f"(r[2]), "=f"(r[3]) : "r"(a) : "memory");
+template <> __device__ __forceinline__ void lds<4>(F2 (&r)[2], uint32_t a) {
+  asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(r[0].v), "=l"(r[1].v) : "r"(a) : "memory");
 }
-__device__ __forceinline__ float lds1(uint32_t a) {
-  float r;
-  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(a) : "memory");
-  return r;
+template <int V> __device__ __forceinline__ void sts(uint32_t a, const F2 (&r)[V / 2]);
+template <> __device__ __forceinline__ void sts<2>(uint32_t a, const F2 (&r)[1]) {
+  asm volatile("st.shared.b64 [%0], %1;" ::"r"(a), "l"(r[0].v) : "memory");
 }
-template <int V> __device__ __forceinline__ void sts(uint32_t a, const float (&r)[V]);
-template <> __device__ __forceinline__ void sts<2>(uint32_t a, const float (&r)[2]) {
-  asm volatile("st.shared.v2.f32 [%0], {%1,%2};" ::"r"(a), "f"(r[0]), "f"(r[1]) : "memory");
-}
-template <> __device__ __forceinline__ void sts<4>(uint32_t a, const float (&r)[4]) {
-  asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]) : "memory");
+template <> __device__ __forceinline__ void sts<4>(uint32_t a, const F2 (&r)[2]) {
+  asm volatile("st.shared.v2.b64 [%0], {%1,%2};" ::"r"(a), "l"(r[0].v), "l"(r[1].v) : "memory");
 }
 // asynchronous store into the shared memory of another CTA of the cluster (addresses from mapa_u32); the bytes are
 // counted on an mbarrier of THAT CTA, whose threads wait on it: no fence on either side
-template <int V> __device__ __forceinline__ void st_async(uint32_t a, const float (&r)[V], uint32_t bar);
-template <> __device__ __forceinline__ void st_async<2>(uint32_t a, const float (&r)[2], uint32_t bar) {
-  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1,%2}, [%3];"
-               ::"r"(a), "f"(r[0]), "f"(r[1]), "r"(bar) : "memory");
+template <int V> __device__ __forceinline__ void st_async(uint32_t a, const F2 (&r)[V / 2], uint32_t bar);
+template <> __device__ __forceinline__ void st_async<2>(uint32_t a, const F2 (&r)[1], uint32_t bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];"
+               ::"r"(a), "l"(r[0].v), "r"(bar) : "memory");
 }
-template <> __device__ __forceinline__ void st_async<4>(uint32_t a, const float (&r)[4], uint32_t bar) {
-  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1,%2,%3,%4}, [%5];"
-               ::"r"(a), "f"(r[0]), "f"(r[1]), "f"(r[2]), "f"(r[3]), "r"(bar) : "memory");
+template <> __device__ __forceinline__ void st_async<4>(uint32_t a, const F2 (&r)[2], uint32_t bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1,%2}, [%3];"
+               ::"r"(a), "l"(r[0].v), "l"(r[1].v), "r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
@@ -153,18 +146,21 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
 // streaming global access for the spins: each value is touched once per sweep
-template <int V> __device__ __forceinline__ void ldg(float (&r)[V], const float* p) {
-  const typename VT<V>::type t = __ldcs(reinterpret_cast<const typename VT<V>::type*>(p));
-  const float* f = reinterpret_cast<const float*>(&t);
-#pragma unroll
-  for (int e = 0; e < V; ++e) r[e] = f[e];
+template <int V> __device__ __forceinline__ void ldg(F2 (&r)[V / 2], const float* p);
+template <> __device__ __forceinline__ void ldg<2>(F2 (&r)[1], const float* p) {
+  const float2 t = __ldcs(reinterpret_cast<const float2*>(p));
+  r[0] = make_f2(t.x, t.y);
 }
-template <int V> __device__ __forceinline__ void stg(float* p, const float (&r)[V]) {
-  typename VT<V>::type t;
-  float* f = reinterpret_cast<float*>(&t);
-#pragma unroll
-  for (int e = 0; e < V; ++e) f[e] = r[e];
-  __stcs(reinterpret_cast<typename VT<V>::type*>(p), t);
+template <> __device__ __forceinline__ void ldg<4>(F2 (&r)[2], const float* p) {
+  const float4 t = __ldcs(reinterpret_cast<const float4*>(p));
+  r[0] = make_f2(t.x, t.y); r[1] = make_f2(t.z, t.w);
+}
+template <int V> __device__ __forceinline__ void stg(float* p, const F2 (&r)[V / 2]);
+template <> __device__ __forceinline__ void stg<2>(float* p, const F2 (&r)[1]) {
+  __stcs(reinterpret_cast<float2*>(p), make_float2(f2_lo(r[0]), f2_hi(r[0])));
+}
+template <> __device__ __forceinline__ void stg<4>(float* p, const F2 (&r)[2]) {
+  __stcs(reinterpret_cast<float4*>(p), make_float4(f2_lo(r[0]), f2_hi(r[0]), f2_lo(r[1]), f2_hi(r[1])));
 }
 
 template <int L, int YS, int V, int G> struct Cfg {
@@ -217,10 +213,12 @@ struct Th {
   int edge;                   // HALO: -1 = lowest row of the strip, +1 = highest row, 0 = interior
   uint32_t row, rowp, rowm;   // byte offsets inside a shared [y][j] array: own row, row y+1, row y-1 at j0
   uint32_t row0;              // own row at j0 inside an array without halo rows (ring C0, J/H arrays)
-  uint32_t jedge0;            // J/H arrays: own row at j0-1 (periodic)
   uint32_t jym0, jym1;        // J/H arrays: offset of row y-1 at j0 relative to the OTHER colour's Jy array, for the colour-0 /
                               // colour-1 update (strips: the lowest row reads the halo rows at the end of the ring slot)
-  uint32_t edge0, edge1;      // own row at j0-1 and j0+V (periodic): the x neighbour outside the thread's V sites
+  int lane_prev, lane_next;   // lanes of the threads that own the sites left / right of this thread's V sites in the same row
+                              // (periodic; a row is TPR consecutive lanes of one warp): the x neighbour outside the thread's
+                              // own sites is one of THEIR registers and travels by shuffle
+  uint32_t lanes;             // shuffle mask: the lanes of this warp that exist
   uint32_t halo;              // HALO edge threads: byte offset of the halo row they fill (== rowm or rowp)
   uint32_t push;              // HALO edge threads: cluster address of X0[0], component 0, halo row at j0 in the neighbour CTA
   uint32_t push_bar;          // HALO edge threads: cluster address of the neighbour CTA's halo mbarrier of X0[0]
@@ -243,79 +241,89 @@ struct JAddr {
 };
 
 // Local field of V sites of one colour in plane zp, accumulated in the order H, x+, x-, y+, y-, z+, z-
-// (DESIGN.md §3.1), then the move.  `q` = the thread's own column of the other colour in this plane,
-// `xs` = shared-memory half-plane of the other colour in this plane (rows y+-1 and the x edge),
-// `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1.  CSB / CJB = byte strides between the
-// component arrays of a shared spin half-plane / between the arrays of a shared J/H plane.
+// (DESIGN.md §3.1), then the move; two sites per packed operation (hsg_math.cuh).  `q` = the thread's own column of the
+// other colour in this plane, `xs` = shared-memory half-plane of the other colour in this plane (rows y+-1),
+// `zlo`/`zhi` = own column of the other colour in planes zp-1 / zp+1.  The x neighbours of compact site j are the other
+// colour's sites j-1+off and j+off of the same row: inside the thread's own V sites they are its registers `q`, the one
+// outside is a register of the neighbouring lane (shuffle).  CSB / CJB = byte strides between the component arrays of a
+// shared spin half-plane / between the arrays of a shared J/H plane.
 // EN = 0: move only; 1: also accumulate s_i.H_i and s_i of the NEW spin (colour 0 in the final sweep);
 // 2: s_i.h_i instead, the whole local field (colour 1 in the final sweep, when all its neighbours already hold their
 // final values: every bond of the lattice once).
 template <uint32_t CSB, uint32_t CJB, int V, bool HB, int EN>
-__device__ __forceinline__ void update_sites(float (&out)[3][V], const float (&own)[3][V], const float (&q)[3][V],
-                                             const float (&zlo)[3][V], const float (&zhi)[3][V], uint32_t xs,
+__device__ __forceinline__ void update_sites(F2 (&out)[3][V / 2], const F2 (&own)[3][V / 2], const F2 (&q)[3][V / 2],
+                                             const F2 (&zlo)[3][V / 2], const F2 (&zhi)[3][V / 2], uint32_t xs,
                                              const JAddr& ja, const Th& th, int off, const HbPar& hp, uint32_t site0, EAcc& ea) {
-  const uint32_t edge = off ? th.edge1 : th.edge0;
-  float Jxp[V], Jxm[V], Jyp[V], Jym[V], Jzp[V], Jzm[V];
+  constexpr int NP = V / 2;
+  const bool up = off != 0;
+  const int src = up ? th.lane_next : th.lane_prev;        // the lane that owns the x neighbour outside this thread's sites
+  // pair p of an array shifted by one site: towards higher j (x+ neighbours when off = 1), towards lower j (x- when off = 0)
+  auto shifted = [&](const F2 (&v)[NP], float outside, int p) {
+    const float lo = up ? f2_hi(v[p]) : (p > 0 ? f2_hi(v[p > 0 ? p - 1 : 0]) : outside);
+    const float hi = up ? (p + 1 < NP ? f2_lo(v[p + 1 < NP ? p + 1 : 0]) : outside) : f2_lo(v[p]);
+    return make_f2(lo, hi);
+  };
+  F2 Jxp[NP], Jxm[NP], Jyp[NP], Jym[NP], Jzp[NP], Jzm[NP];
   lds<V>(Jxp, ja.own_xy + th.row0);
   lds<V>(Jyp, ja.own_xy + CJB + th.row0);
   lds<V>(Jzp, ja.own_z + th.row0);
   {
-    float t[V];
+    F2 t[NP];
     lds<V>(t, ja.oth_xy + th.row0);
-    const float te = lds1(ja.oth_xy + th.jedge0);
+    // the bond from x-1 is the +x coupling stored at the other colour's site j-1+off: the thread's own t[] when off = 1
+    const float te = __shfl_sync(th.lanes, f2_hi(t[NP - 1]), th.lane_prev);
 #pragma unroll
-    for (int e = 0; e < V; ++e) Jxm[e] = off ? t[e] : (e > 0 ? t[e > 0 ? e - 1 : 0] : te);
+    for (int p = 0; p < NP; ++p) Jxm[p] = up ? t[p] : shifted(t, te, p);
   }
   lds<V>(Jym, ja.oth_xy + CJB + ja.ym);
   lds<V>(Jzm, ja.oth_z + th.row0);
-  float h[3][V];
-  float Hs[3][V];
-  const uint32_t xs_p = xs + th.rowp, xs_m = xs + th.rowm, xs_e = xs + edge;
+  F2 h[3][NP], Hs[3][NP];
+  const uint32_t xs_p = xs + th.rowp, xs_m = xs + th.rowm;
 #pragma unroll
   for (int mu = 0; mu < 3; ++mu) {
-    float Hm[V], yp[V], ym[V];
+    F2 Hm[NP], yp[NP], ym[NP];
     lds<V>(Hm, ja.own_h + mu * CJB + th.row0);
     lds<V>(yp, xs_p + mu * CSB);
     lds<V>(ym, xs_m + mu * CSB);
-    const float se = lds1(xs_e + mu * CSB);
+    const float se = __shfl_sync(th.lanes, up ? f2_lo(q[mu][0]) : f2_hi(q[mu][NP - 1]), src);
 #pragma unroll
-    for (int e = 0; e < V; ++e) {
-      const float sxp = off ? (e + 1 < V ? q[mu][e + 1 < V ? e + 1 : 0] : se) : q[mu][e];
-      const float sxm = off ? q[mu][e] : (e > 0 ? q[mu][e > 0 ? e - 1 : 0] : se);
-      float acc = Hm[e];
-      acc = __fmaf_rn(Jxp[e], sxp, acc);
-      acc = __fmaf_rn(Jxm[e], sxm, acc);
-      acc = __fmaf_rn(Jyp[e], yp[e], acc);
-      acc = __fmaf_rn(Jym[e], ym[e], acc);
-      acc = __fmaf_rn(Jzp[e], zhi[mu][e], acc);
-      acc = __fmaf_rn(Jzm[e], zlo[mu][e], acc);
-      h[mu][e] = acc;
-      if (EN == 1) Hs[mu][e] = Hm[e];
+    for (int p = 0; p < NP; ++p) {
+      const F2 sh = shifted(q[mu], se, p);
+      const F2 sxp = up ? sh : q[mu][p];
+      const F2 sxm = up ? q[mu][p] : sh;
+      F2 acc = Hm[p];
+      acc = fma_rn(Jxp[p], sxp, acc);
+      acc = fma_rn(Jxm[p], sxm, acc);
+      acc = fma_rn(Jyp[p], yp[p], acc);
+      acc = fma_rn(Jym[p], ym[p], acc);
+      acc = fma_rn(Jzp[p], zhi[mu][p], acc);
+      acc = fma_rn(Jzm[p], zlo[mu][p], acc);
+      h[mu][p] = acc;
+      if (EN == 1) Hs[mu][p] = Hm[p];
     }
   }
-  // heat bath: one Philox call per pair of sites (e, e+1), e even: counter word 0 = the site with even compact index
-  // (j0 is a multiple of V), which takes output words 0, 1; its partner takes words 2, 3
-  uint32_t wa[V], wb[V];
-  if (HB) {
 #pragma unroll
-    for (int e = 0; e < V; e += 2)
-      philox4x32_10(site0 + 2u * (uint32_t)e, hp.c1, hp.sysid, hp.c3, hp.key.k0, hp.key.k1, wa[e], wb[e], wa[e + 1], wb[e + 1]);
-  }
-#pragma unroll
-  for (int e = 0; e < V; ++e) {
-    const Vec3 hv = {h[0][e], h[1][e], h[2][e]};
-    Vec3 s;
+  for (int p = 0; p < NP; ++p) {
+    const V3<F2> hv = {h[0][p], h[1][p], h[2][p]};
+    V3<F2> s;
     if (HB) {
-      s = hb_draw(hv, hp.beta, u01(wa[e]), u01(wb[e]));
+      // heat bath: one Philox call per pair of sites (e, e+1), e even: counter word 0 = the site with even compact index
+      // (j0 is a multiple of V), which takes output words 0, 1; its partner takes words 2, 3
+      uint32_t w0, w1, w2, w3;
+      philox4x32_10(site0 + 4u * (uint32_t)p, hp.c1, hp.sysid, hp.c3, hp.key.k0, hp.key.k1, w0, w1, w2, w3);
+      s = hb_draw(hv, hp.beta, make_f2(u01(w0), u01(w2)), make_f2(u01(w1), u01(w3)));
     } else {
-      const Vec3 sv = {own[0][e], own[1][e], own[2][e]};
+      const V3<F2> sv = {own[0][p], own[1][p], own[2][p]};
       s = or_reflect(sv, hv);
     }
-    out[0][e] = s.x; out[1][e] = s.y; out[2][e] = s.z;
+    out[0][p] = s.x; out[1][p] = s.y; out[2][p] = s.z;
     if (EN >= 1) {
-      const Vec3 f = {EN == 2 ? h[0][e] : Hs[0][e], EN == 2 ? h[1][e] : Hs[1][e], EN == 2 ? h[2][e] : Hs[2][e]};
-      ea.e += (double)dot3(s, f);
-      ea.mx += (double)s.x; ea.my += (double)s.y; ea.mz += (double)s.z;
+      const V3<F2> f = {EN == 2 ? h[0][p] : Hs[0][p], EN == 2 ? h[1][p] : Hs[1][p], EN == 2 ? h[2][p] : Hs[2][p]};
+      const F2 sf = dot3(s, f);
+      ea.e += (double)f2_lo(sf); ea.e += (double)f2_hi(sf);
+      ea.mx += (double)f2_lo(s.x); ea.mx += (double)f2_hi(s.x);
+      ea.my += (double)f2_lo(s.y); ea.my += (double)f2_hi(s.y);
+      ea.mz += (double)f2_lo(s.z); ea.mz += (double)f2_hi(s.z);
     }
   }
 }
@@ -427,7 +435,8 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   constexpr uint32_t CSB = 4u * C::CSS, HPB = 4u * C::HPS, CJB = 4u * C::CSJ, JAB = 4u * C::JA, JBB = 4u * C::CSJ;
   constexpr uint32_t CS0B = 4u * C::CS0, HP0B = 4u * C::HP0;
   constexpr bool HALO = C::HALO;
-  float A[3][V], B[3][V], Cc[3][V], O[3][V], P[3][V], Q[3][V], R[3][V], On[3][V];
+  constexpr int NP = V / 2;
+  F2 A[3][NP], B[3][NP], Cc[3][NP], O[3][NP], P[3][NP], Q[3][NP], R[3][NP], On[3][NP];
   float* Sr = S + th.grow;                             // own column, plane 0, colour 0, component 0
   const float* Sh = S + th.grow_halo;                  // HALO edge threads: the halo row they fetch
 
@@ -454,7 +463,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     cp_async_commit();                                  // an empty group keeps the group count uniform
   };
   // new colour-0 spins of a plane -> X0[par] of this CTA and, from the strip's edge rows, the neighbour CTA's halo row
-  auto publish_x0 = [&](uint32_t par, const float (&v)[3][V]) {
+  auto publish_x0 = [&](uint32_t par, const F2 (&v)[3][NP]) {
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) {
       sts<V>(sm.x0 + par * HPB + mu * CSB + th.row, v[mu]);
@@ -481,7 +490,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   for (int mu = 0; mu < 3; ++mu) {
     ldg<V>(A[mu], Sr + (L - 1) * PS + HP + mu * CS);
 #pragma unroll
-    for (int e = 0; e < V; ++e) { P[mu][e] = 0.0f; Q[mu][e] = 0.0f; O[mu][e] = 0.0f; On[mu][e] = 0.0f; }
+    for (int e = 0; e < NP; ++e) { P[mu][e].v = 0ull; Q[mu][e].v = 0ull; O[mu][e].v = 0ull; On[mu][e].v = 0ull; }
   }
   cp_async_wait<C::DS>();
 #pragma unroll
@@ -523,7 +532,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     if (k >= 2) {     // colour 1 of plane k-1
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * (k - 1)));
       const JAddr ja = {ak1 + 5 * CJB, ak1 + 7 * CJB, ak1 + 8 * CJB, ak1, bk2, th.jym1};
-      float N1[3][V];
+      F2 N1[3][NP];
       update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + (k - 1) * PS + HP + mu * CS, N1[mu]);
@@ -532,7 +541,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
-      for (int e = 0; e < V; ++e) { A[mu][e] = B[mu][e]; B[mu][e] = Cc[mu][e]; P[mu][e] = Q[mu][e]; Q[mu][e] = R[mu][e]; }
+      for (int e = 0; e < NP; ++e) { A[mu][e] = B[mu][e]; B[mu][e] = Cc[mu][e]; P[mu][e] = Q[mu][e]; Q[mu][e] = R[mu][e]; }
   }
   cp_async_wait<0>();                                   // only empty groups are left
   // tail: colour 1 of plane L-1 (step L) and of plane 0 (step L+1); their z+ neighbours are the new colour-0
@@ -545,7 +554,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
-      for (int e = 0; e < V; ++e) R[mu][e] = On[mu][e];
+      for (int e = 0; e < NP; ++e) R[mu][e] = On[mu][e];
     if (kk == 0) arm_halo(0u);
     step_wait<C>();
     if (kk == 0) {
@@ -560,7 +569,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     const int z1 = kk == 0 ? L - 1 : 0;
     const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * z1));
     const JAddr ja = {a1 + 5 * CJB, a1 + 7 * CJB, a1 + 8 * CJB, a1, b2, th.jym1};
-    float N1[3][V];
+    F2 N1[3][NP];
     update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + z1 * PS + HP + mu * CS, N1[mu]);
@@ -569,7 +578,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu)
 #pragma unroll
-      for (int e = 0; e < V; ++e) { A[mu][e] = B[mu][e]; P[mu][e] = Q[mu][e]; Q[mu][e] = R[mu][e]; }
+      for (int e = 0; e < NP; ++e) { A[mu][e] = B[mu][e]; P[mu][e] = Q[mu][e]; Q[mu][e] = R[mu][e]; }
   }
 }
 
@@ -624,15 +633,21 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
     th.rowm = 4u * (uint32_t)(((ly == 0) ? L - 1 : ly - 1) * C::Lh + th.j0);
     th.edge = 0; th.grow_halo = 0; th.halo = 0; th.push = 0; th.push_bar = 0;
   }
-  th.jedge0 = 4u * (uint32_t)(ly * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1));
   if (C::HALO && ly == 0) {       // row y0-1 of the other colour's Jy: halo rows behind the 11 arrays of the ring-A slot
     th.jym0 = 4u * (uint32_t)((11 - 6) * C::CSJ + C::Lh + th.j0);    // colour-0 update reads colour-1 Jy (array 6), halo row 1
     th.jym1 = 4u * (uint32_t)((11 - 1) * C::CSJ + th.j0);            // colour-1 update reads colour-0 Jy (array 1), halo row 0
   } else {
     th.jym0 = th.jym1 = 4u * (uint32_t)(((ly == 0) ? L - 1 : ly - 1) * C::Lh + th.j0);
   }
-  th.edge0 = 4u * (uint32_t)((ly + HR) * C::Lh + ((th.j0 == 0) ? C::Lh - 1 : th.j0 - 1));
-  th.edge1 = 4u * (uint32_t)((ly + HR) * C::Lh + ((th.j0 + V == C::Lh) ? 0 : th.j0 + V));
+  {
+    // the TPR threads of a row are consecutive lanes of one warp (TPR divides 32)
+    static_assert(32 % C::TPR == 0 || C::TPR % 32 == 0, "a row occupies whole warps or a power-of-two part of one");
+    static_assert(C::TPR <= 32, "a row must fit one warp: its x neighbours travel by shuffle");
+    const int lane = (int)(threadIdx.x & 31u), first = lane & ~(C::TPR - 1);
+    th.lane_prev = first | ((lane - 1) & (C::TPR - 1));
+    th.lane_next = first | ((lane + 1) & (C::TPR - 1));
+    th.lanes = C::NT >= 32 ? 0xffffffffu : ((1u << (C::NT & 31)) - 1u);
+  }
 
   const Geom& g = a.g;
   const int slot = group * G + gs;                      // G consecutive slots of one sample
