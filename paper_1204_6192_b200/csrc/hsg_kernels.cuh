@@ -503,6 +503,14 @@ __global__ void selftest_arith_kernel(PhiloxKey key, unsigned long long n, unsig
     // the reciprocals +-1/b (the move uses them for 1/|h| and -1/(sigma + n_z)), and the packed instantiation of all three
     if (__float_as_uint(rcp_rn<float, false>(x)) != __float_as_uint(__fdiv_rn(1.0f, x))) ++bad_div;
     if (__float_as_uint(rcp_rn<float, true>(b2)) != __float_as_uint(__fdiv_rn(-1.0f, b2))) ++bad_div;
+    // divisors whose mantissa is all ones: the one exceptional case of the Newton scheme, where the last correction lands
+    // on the rounded quotient only for a good enough seed (tests/test_device_math_on_host.py) — the hardware's must be
+    const float b3 = __uint_as_float(__float_as_uint(b) | 0x007FFFFFu), x3 = fabsf(b3);
+    const float q3 = __fdiv_rn(a, b3);
+    if (fabsf(q3) >= 1.2e-38f && fabsf(q3) <= 3.0e38f && __float_as_uint(div_rn(a, b3)) != __float_as_uint(q3)) ++bad_div;
+    if (__float_as_uint(rcp_rn<float, false>(x3)) != __float_as_uint(__fdiv_rn(1.0f, x3))) ++bad_div;
+    if (__float_as_uint(div_rn(a2, 1.99999988079071044921875f)) != __float_as_uint(__fdiv_rn(a2, 1.99999988079071044921875f))) ++bad_div;
+    if ((i & 0xFFFFull) == 0 && __float_as_uint(rcp_rn<float, true>(1.99999988079071044921875f)) != 0xBF000001u) ++bad_div;   // -1/(2 - 2^-23)
     const F2 qp = div_rn(make_f2(a, a2), make_f2(b, b2));
     if (fabsf(q2) >= 1.2e-38f && fabsf(q2) <= 3.0e38f && __float_as_uint(f2_lo(qp)) != __float_as_uint(q2)) ++bad_div;
     if (__float_as_uint(f2_hi(qp)) != __float_as_uint(__fdiv_rn(a2, b2))) ++bad_div;
