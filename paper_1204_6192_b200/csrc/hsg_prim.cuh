@@ -2,7 +2,7 @@
 // binary32 operations on one value (float) or on two values at once (F2, the packed f32x2 instructions of sm_100), the
 // approximate reciprocal / reciprocal-square-root seeds.  Everything in hsg_math.cuh is plain C++ over these and over
 // the compiler's __fmaf_rn-style intrinsics, so that tests/test_device_math_on_host.py can compile the very same move
-// templates for the host, against a host restatement of THIS file, and compare them with the oracle bit for bit.
+// templates for the host, against a host restatement of THIS file, and compare them with the serial reference bit for bit.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
