@@ -174,7 +174,8 @@ def main_ours(args, cfg, temps):
     J = hsg_inputs.couplings(L, D, cfg["seed"], off)
     H = hsg_inputs.gaussian_field(L, D, cfg["h_r"], cfg["seed"], off) if cfg["h_r"] > 0 else None
 
-    eng = hsg.hsg_create(L, D, O, temps, cfg["seed"], sample_offset=off, kernel=args.kernel)
+    flags = hsg.HSG_FLAG_FAST_MATH if args.fast_math else 0   # a separately reported VARIANT, never the default
+    eng = hsg.hsg_create(L, D, O, temps, cfg["seed"], sample_offset=off, kernel=args.kernel, flags=flags)
     if args.no_fuse_energy:
         eng.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
     eng.set_disorder(J, H)
@@ -295,7 +296,7 @@ def main_ours(args, cfg, temps):
         for k in range(K):
             st = torch.cuda.Stream()
             with torch.cuda.stream(st):
-                e = hsg.hsg_create(L, Ds, O, temps, cfg["seed"], sample_offset=off + k * Ds, stream=st, kernel=args.kernel)
+                e = hsg.hsg_create(L, Ds, O, temps, cfg["seed"], sample_offset=off + k * Ds, stream=st, kernel=args.kernel, flags=flags)
                 if args.no_fuse_energy:
                     e.set_option(hsg.HSG_OPT_FUSE_ENERGY, 0)
                 sl = slice(k * Ds, (k + 1) * Ds)
@@ -389,6 +390,8 @@ def main_ours(args, cfg, temps):
                                    f"{n_or} OR + {n_hb} HB + PT{' + measure' if measure else ''} per step",
                        "L": L, "n_samples_per_gpu": D, "n_replicas": O, "n_temps": T, "n_or": n_or, "n_hb": n_hb,
                        "parallelism": f"samples sharded over {world} GPU(s), no collective", "sweep_kernel": kernel,
+                       "arithmetic": "fast-math heat-bath VARIANT (HSG_FLAG_FAST_MATH; not the parity arithmetic)" if args.fast_math
+                                     else "reference (bit-exact against the oracle)",
                        "l2": "state (spins) far larger than L2; no flush needed"},
             "ns_per_update_sweeps_only": ns_sweeps, "roofline": roofline,
             "cpu_baseline": {"value": ns_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": text},
@@ -411,6 +414,7 @@ def main():
     ap.add_argument("--samples", type=int, default=None, help="override the number of disorder samples per GPU")
     ap.add_argument("--n-or", type=int, default=None, help="override the over-relaxation sweeps per step (OR-only / HB-only timing points)")
     ap.add_argument("--n-hb", type=int, default=None, help="override the heat-bath sweeps per step")
+    ap.add_argument("--fast-math", action="store_true", help="time the fast-math heat-bath variant (HSG_FLAG_FAST_MATH) instead of the reference arithmetic")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-shards", type=int, default=0, help="sample shards (contexts + streams) of the end-to-end round; 0 = 8 or 4 if they divide the samples")
     ap.add_argument("--no-measure", action="store_true")

@@ -65,6 +65,17 @@ enum {
                               reduction kernel.  Values agree to fp64 summation order (~1e-15 relative). */
 };
 
+/* hsg_desc.flags */
+enum {
+  HSG_FLAG_FAST_MATH = 1   /* VARIANT of the heat-bath update (Table 1 rows PAPER.md:211,215,218: "fast_math"): the
+                              same draw — same uniforms, inverse CDF and frame — with the correctly rounded divisions, square
+                              roots and fixed series of DESIGN.md §3.3-3.4 replaced by the special-function unit's approximations
+                              (rsqrt, ex2, lg2, rcp, sqrt, sin, cos).  Over-relaxation, energies, swaps and measurements are
+                              unchanged.  Runs are still deterministic, but NOT bit-identical to the reference arithmetic: one
+                              heat-bath update from equal inputs differs per spin component by at most
+                              sqrt(2e-6 (1 + 1/a)), a = beta |h| (median ~ 1e-6 (1 + 1/a)); DESIGN.md §3.9. */
+};
+
 typedef struct hsg_ctx hsg_ctx; /* opaque, host side */
 
 typedef struct {

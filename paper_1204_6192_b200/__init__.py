@@ -20,6 +20,7 @@ from . import _build
 HSG_OK, HSG_EINVAL, HSG_ESTATE, HSG_EUNSUPPORTED, HSG_ECUDA = 0, -1, -2, -3, -4
 HSG_KERNEL_AUTO, HSG_KERNEL_GENERIC, HSG_KERNEL_ZMARCH = 0, 1, 2
 HSG_OPT_SWEEP_KERNEL, HSG_OPT_FUSE_ENERGY = 1, 2
+HSG_FLAG_FAST_MATH = 1
 KERNELS = {"auto": HSG_KERNEL_AUTO, "generic": HSG_KERNEL_GENERIC, "zmarch": HSG_KERNEL_ZMARCH}
 
 # every symbol include/hsg.h declares (tests check that the library exports each of them)
@@ -104,10 +105,10 @@ def hsg_xi_second_moment(chi_0, chi_kmin, L) -> float:
     return xi.value
 
 
-def hsg_query_bytes(L, n_samples, n_replicas, temps, seed=0, sample_offset=0):
+def hsg_query_bytes(L, n_samples, n_replicas, temps, seed=0, sample_offset=0, flags=0):
     temps = np.ascontiguousarray(temps, dtype=np.float32)
     d = hsg_desc(int(L), int(n_samples), int(n_replicas), len(temps), temps.ctypes.data_as(C.POINTER(C.c_float)),
-                 int(seed), int(sample_offset), 0)
+                 int(seed), int(sample_offset), int(flags))
     a, b = C.c_size_t(0), C.c_size_t(0)
     rc = lib().hsg_query_bytes(C.byref(d), C.byref(a), C.byref(b))
     if rc != HSG_OK:
@@ -130,7 +131,7 @@ def _on_device(method):
 class Hsg:
     """One hsg context over torch-owned device buffers.  Methods mirror the C calls (hsg_<name>)."""
 
-    def __init__(self, L, n_samples, n_replicas, temps, seed, sample_offset=0, device=None, stream=None, kernel="auto"):
+    def __init__(self, L, n_samples, n_replicas, temps, seed, sample_offset=0, device=None, stream=None, kernel="auto", flags=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("hsg needs a CUDA device: there is no CPU fallback")
@@ -142,7 +143,7 @@ class Hsg:
         self.N = self.L ** 3
         self.P = self.O * (self.O - 1) // 2
         self._desc = hsg_desc(self.L, self.D, self.O, self.T, self.temps.ctypes.data_as(C.POINTER(C.c_float)),
-                              int(seed), int(sample_offset), 0)
+                              int(seed), int(sample_offset), int(flags))
         nb_state, nb_scratch = C.c_size_t(0), C.c_size_t(0)
         rc = lib().hsg_query_bytes(C.byref(self._desc), C.byref(nb_state), C.byref(nb_scratch))
         if rc != HSG_OK:

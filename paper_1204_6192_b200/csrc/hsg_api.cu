@@ -61,7 +61,7 @@ ScratchLayout scratch_layout(const Geom& g) {
 int check_desc(const hsg_desc* d) {
   if (!d || !d->temps_host) return HSG_EINVAL;
   if (d->L < 2 || (d->L & 1) || d->n_samples < 1 || d->n_replicas < 1 || d->n_temps < 1) return HSG_EINVAL;
-  if (d->flags != 0) return HSG_EINVAL;
+  if (d->flags & ~(uint32_t)HSG_FLAG_FAST_MATH) return HSG_EINVAL;
   for (int t = 0; t < d->n_temps; ++t) {
     if (!(d->temps_host[t] > 0.0f) || !std::isfinite(d->temps_host[t])) return HSG_EINVAL;
     if (t > 0 && !(d->temps_host[t] > d->temps_host[t - 1])) return HSG_EINVAL;
@@ -105,6 +105,7 @@ struct hsg_ctx {
   int sm_count;                 // its number of SMs (grid sizing of the sweep kernels)
   int sweep_kernel_opt;
   bool fuse_energy;             // zmarch: reduce E and m in the final sweep of every hsg_sweep call
+  bool fast_math;               // HSG_FLAG_FAST_MATH: heat-bath sweeps draw with the special-function unit
   const char* last_kernel;
   unsigned long long launches;
   std::string err;
@@ -163,6 +164,7 @@ int hsg_create(const hsg_desc* desc, void* dev_state, size_t state_bytes, void* 
   c->diag_on = false; c->diag_passes = 0;
   c->k_hb = 0; c->k_pt = 0; c->have_disorder = false; c->have_spins = false; c->energy_valid = false;
   c->sweep_kernel_opt = HSG_KERNEL_AUTO; c->fuse_energy = true; c->last_kernel = "none"; c->launches = 0;
+  c->fast_math = (desc->flags & HSG_FLAG_FAST_MATH) != 0;
 
   // small host-computed tables: beta_t = (float)(1.0/(double)T_t); cos/sin(2 pi x / L) in fp64
   std::vector<float> beta(g.T);
@@ -257,9 +259,10 @@ static int launch_generic_sweep(hsg_ctx* ctx, bool hb) {
   const long long n = (long long)g.R * g.L * g.L * (g.Lh / V);
   for (int colour = 0; colour < 2; ++colour) {
     const unsigned nb = blocks_for(n);
-    if (V == 4) { if (hb) sweep_generic_kernel<4, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<4, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
-    else if (V == 2) { if (hb) sweep_generic_kernel<2, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<2, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
-    else { if (hb) sweep_generic_kernel<1, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<1, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
+    const bool fm = hb && ctx->fast_math;
+    if (V == 4) { if (fm) sweep_generic_kernel<4, true, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else if (hb) sweep_generic_kernel<4, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<4, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
+    else if (V == 2) { if (fm) sweep_generic_kernel<2, true, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else if (hb) sweep_generic_kernel<2, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<2, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
+    else { if (fm) sweep_generic_kernel<1, true, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else if (hb) sweep_generic_kernel<1, true><<<nb, kThreads, 0, ctx->stream>>>(a, colour); else sweep_generic_kernel<1, false><<<nb, kThreads, 0, ctx->stream>>>(a, colour); }
     HSG_LAUNCHED(ctx);
   }
   return HSG_OK;
@@ -276,7 +279,7 @@ int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
   if (kernel == HSG_KERNEL_ZMARCH) {
     // the final sweep of the call also reduces E and m of every slot
     ZmarchArgs a{ctx->g, ctx->spins, ctx->jh, ctx->temp_of_slot, ctx->beta, ctx->key, ctx->k_hb, n_or, n_hb,
-                 ctx->fuse_energy ? ctx->e_slot : nullptr, ctx->m_slot};
+                 ctx->fuse_energy ? ctx->e_slot : nullptr, ctx->m_slot, ctx->fast_math ? 1 : 0};
     int n_launch = 0;
     const cudaError_t e = zmarch_launch(a, ctx->stream, &n_launch, ctx->sm_count);
     ctx->launches += (unsigned long long)n_launch;

@@ -166,8 +166,8 @@ __device__ __forceinline__ void local_field_global(const Geom& g, const float* _
 
 // Each thread updates V consecutive compact sites of colour `colour` in one row (y,z) of one slot.
 // Neighbours are read straight from global memory (L1/L2 provide the reuse).  The field is accumulated
-// in the order H, x+, x-, y+, y-, z+, z- (DESIGN.md §3.1).
-template <int V, bool HB>
+// in the order H, x+, x-, y+, y-, z+, z- (DESIGN.md §3.1).  FM: the fast-math variant of the heat-bath draw (HSG_FLAG_FAST_MATH).
+template <int V, bool HB, bool FM = false>
 __global__ void __launch_bounds__(kThreads) sweep_generic_kernel(SweepArgs a, int colour) {
   const Geom& g = a.g;
   const int L = g.L, Lh = g.Lh;
@@ -221,7 +221,7 @@ __global__ void __launch_bounds__(kThreads) sweep_generic_kernel(SweepArgs a, in
 #pragma unroll
     for (int e = 0; e < V; ++e) {
       const Vec3 hv = { h[0][e], h[1][e], h[2][e] };
-      const Vec3 s = hb_draw(hv, beta, u01(wa[e]), u01(wb[e]));
+      const Vec3 s = FM ? hb_draw_fast(hv, beta, u01(wa[e]), u01(wb[e])) : hb_draw(hv, beta, u01(wa[e]), u01(wb[e]));
       out[0].v[e] = s.x; out[1].v[e] = s.y; out[2].v[e] = s.z;
     }
   } else {

@@ -36,4 +36,14 @@ __device__ __forceinline__ F2 neg(F2 a) { return make_f2(-f2_lo(a), -f2_hi(a)); 
 __device__ __forceinline__ float rcp_approx(float b) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b)); return r; }
 __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
+
+// special-function unit approximations of the fast-math heat-bath VARIANT only (HSG_FLAG_FAST_MATH, hb_draw_fast): PTX ISA
+// error bounds — ex2: 2^-22 relative; lg2: 2^-22 absolute for arguments in (0.5, 2), 2^-22 relative otherwise;
+// sin, cos: 2^-20.5 absolute on [-2 pi, 2 pi]; sqrt: 2^-23 relative
+__device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sin_approx(float x) { float y; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float cos_approx(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
 }  // namespace hsg

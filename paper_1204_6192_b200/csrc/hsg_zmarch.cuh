@@ -250,7 +250,8 @@ struct JAddr {
 // EN = 0: move only; 1: also accumulate s_i.H_i and s_i of the NEW spin (colour 0 in the final sweep);
 // 2: s_i.h_i instead, the whole local field (colour 1 in the final sweep, when all its neighbours already hold their
 // final values: every bond of the lattice once).
-template <uint32_t CSB, uint32_t CJB, int V, bool HB, int EN>
+// FM: the heat-bath draw is the fast-math variant hb_draw_fast (HSG_FLAG_FAST_MATH), otherwise the reference arithmetic.
+template <uint32_t CSB, uint32_t CJB, int V, bool HB, int EN, bool FM>
 __device__ __forceinline__ void update_sites(F2 (&out)[3][V / 2], const F2 (&own)[3][V / 2], const F2 (&q)[3][V / 2],
                                              const F2 (&zlo)[3][V / 2], const F2 (&zhi)[3][V / 2], uint32_t xs,
                                              const JAddr& ja, const Th& th, int off, const HbPar& hp, uint32_t site0, EAcc& ea) {
@@ -311,7 +312,8 @@ __device__ __forceinline__ void update_sites(F2 (&out)[3][V / 2], const F2 (&own
       // (j0 is a multiple of V), which takes output words 0, 1; its partner takes words 2, 3
       uint32_t w0, w1, w2, w3;
       philox4x32_10(site0 + 4u * (uint32_t)p, hp.c1, hp.sysid, hp.c3, hp.key.k0, hp.key.k1, w0, w1, w2, w3);
-      s = hb_draw(hv, hp.beta, make_f2(u01(w0), u01(w2)), make_f2(u01(w1), u01(w3)));
+      if constexpr (FM) s = hb_draw_fast(hv, hp.beta, make_f2(u01(w0), u01(w2)), make_f2(u01(w1), u01(w3)));
+      else s = hb_draw(hv, hp.beta, make_f2(u01(w0), u01(w2)), make_f2(u01(w1), u01(w3)));
     } else {
       const V3<F2> sv = {own[0][p], own[1][p], own[2][p]};
       s = or_reflect(sv, hv);
@@ -426,7 +428,7 @@ template <class C> __device__ __forceinline__ void step_wait() {
 }
 
 // One full sweep (both colours, all planes) of the G systems of this CTA.
-template <int L, int YS, int V, int G, bool HB, bool EN>
+template <int L, int YS, int V, int G, bool HB, bool EN, bool FM>
 __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ S, const float* __restrict__ jh_d,
                                             const Th& th, const HbPar& hp, int qbase, Stream& st, EAcc& ea,
                                             uint64_t pol_spin, uint64_t pol_jh, uint32_t& hph) {
@@ -522,7 +524,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     {
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * k));
       const JAddr ja = {ak, bk, ak + 2 * CJB, ak + 5 * CJB, ak1 + 7 * CJB, th.jym0};
-      update_sites<CSB, CJB, V, HB, EN ? 1 : 0>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % C::NC1) * HPB, ja, th, off, hp, site0, ea);
+      update_sites<CSB, CJB, V, HB, EN ? 1 : 0, FM>(R, O, B, A, Cc, sm.c1 + (uint32_t)(k % C::NC1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + k * PS + mu * CS, R[mu]);
       step_wait<C>();
@@ -533,7 +535,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
       const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * (k - 1)));
       const JAddr ja = {ak1 + 5 * CJB, ak1 + 7 * CJB, ak1 + 8 * CJB, ak1, bk2, th.jym1};
       F2 N1[3][NP];
-      update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, ja, th, off, hp, site0, ea);
+      update_sites<CSB, CJB, V, HB, EN ? 2 : 0, FM>(N1, A, Q, P, R, sm.x0 + (par ^ 1u) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
       for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + (k - 1) * PS + HP + mu * CS, N1[mu]);
     }
@@ -570,7 +572,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
     const uint32_t site0 = (uint32_t)(2 * th.j0 + off + L * (th.gy + L * z1));
     const JAddr ja = {a1 + 5 * CJB, a1 + 7 * CJB, a1 + 8 * CJB, a1, b2, th.jym1};
     F2 N1[3][NP];
-    update_sites<CSB, CJB, V, HB, EN ? 2 : 0>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, ja, th, off, hp, site0, ea);
+    update_sites<CSB, CJB, V, HB, EN ? 2 : 0, FM>(N1, A, Q, P, R, sm.x0 + (uint32_t)((k - 1) & 1) * HPB, ja, th, off, hp, site0, ea);
 #pragma unroll
     for (int mu = 0; mu < 3; ++mu) stg<V>(Sr + z1 * PS + HP + mu * CS, N1[mu]);
     if (kk == 1) step_end<C, true>();
@@ -582,7 +584,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   }
 }
 
-template <int L, int YS, int V, int G>
+template <int L, int YS, int V, int G, bool FM>
 __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchArgs a) {
   using C = Cfg<L, YS, V, G>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -674,13 +676,13 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
     const bool fin = want_e && s + 1 == n_sweeps;       // the final sweep also reduces E and m
     if (s < a.n_or) {
       hp.c1 = 0; hp.c3 = 0;
-      if (fin) march_sweep<L, YS, V, G, false, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
-      else march_sweep<L, YS, V, G, false, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
+      if (fin) march_sweep<L, YS, V, G, false, true, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
+      else march_sweep<L, YS, V, G, false, false, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
     } else {
       const unsigned long long khb = a.k_hb + (unsigned long long)(s - a.n_or);
       hp.c1 = (uint32_t)(khb & 0xFFFFFFFFull); hp.c3 = counter_hi(khb, DOMAIN_HB);
-      if (fin) march_sweep<L, YS, V, G, true, true>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
-      else march_sweep<L, YS, V, G, true, false>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
+      if (fin) march_sweep<L, YS, V, G, true, true, FM>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
+      else march_sweep<L, YS, V, G, true, false, FM>(sm, S, jh_d, th, hp, s * L, st, ea, pol_spin, pol_jh, hph);
     }
   }
   step_wait<C>();                                        // strips: nobody pushes into this CTA any more
@@ -722,15 +724,15 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
 }  // namespace zm
 
 // ------------------------------------------------------------------------------------------------ host side
-template <int L, int YS, int V, int G>
+template <int L, int YS, int V, int G, bool FM = false>
 inline cudaError_t zmarch_launch_t(const ZmarchArgs& a, cudaStream_t stream) {
   using C = zm::Cfg<L, YS, V, G>;
   // the attribute is per device: set it on every launch (a host-side table lookup) rather than remember per process,
   // so that contexts on several devices of one process work (hsg.h: "distinct contexts are independent")
-  const cudaError_t e = cudaFuncSetAttribute(zm::zmarch_kernel<L, YS, V, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
+  const cudaError_t e = cudaFuncSetAttribute(zm::zmarch_kernel<L, YS, V, G, FM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
   if (e != cudaSuccess) return e;
   if (C::NCL == 1) {
-    zm::zmarch_kernel<L, YS, V, G><<<a.g.R / G, C::NT, C::smem_bytes, stream>>>(a);
+    zm::zmarch_kernel<L, YS, V, G, FM><<<a.g.R / G, C::NT, C::smem_bytes, stream>>>(a);
     return cudaGetLastError();
   }
   cudaLaunchConfig_t cfg = {};
@@ -742,7 +744,7 @@ inline cudaError_t zmarch_launch_t(const ZmarchArgs& a, cudaStream_t stream) {
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = C::NCL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, zm::zmarch_kernel<L, YS, V, G>, a);
+  return cudaLaunchKernelEx(&cfg, zm::zmarch_kernel<L, YS, V, G, FM>, a);
 }
 
 // hsg_sweep(n_or, n_hb) at lattice size L with G systems per CTA: one launch, or (VHB != V and both phases present) an
@@ -761,7 +763,11 @@ inline cudaError_t zmarch_launch_g(const ZmarchArgs& a, cudaStream_t stream, int
     }
     ZmarchArgs h = a;
     h.n_or = 0;
-    return zmarch_launch_t<L, T::YS, T::VHB, G>(h, stream);
+    return a.fast_math ? zmarch_launch_t<L, T::YS, T::VHB, G, true>(h, stream) : zmarch_launch_t<L, T::YS, T::VHB, G>(h, stream);
+  }
+  // (only a launch that holds heat-bath sweeps has a fast-math form: over-relaxation is the reference arithmetic either way)
+  if constexpr (T::VHB == T::V) {
+    if (a.fast_math && a.n_hb > 0) return zmarch_launch_t<L, T::YS, T::V, G, true>(a, stream);
   }
   return zmarch_launch_t<L, T::YS, T::V, G>(a, stream);
 }

@@ -18,6 +18,7 @@ struct ZmarchArgs {
   int n_or, n_hb;
   double* e_slot;               // [R]    energy of every slot after the call, or nullptr
   double* m_slot;               // [R][3] magnetisation of every slot after the call
+  int fast_math;                // heat-bath sweeps use the fast-math variant of the draw (HSG_FLAG_FAST_MATH)
 };
 
 // n_launch receives the number of kernel launches made (0 on error); sm_count = SMs of the current device

@@ -39,6 +39,13 @@ def test_query_bytes_and_descriptor_validation_without_a_gpu():
                 (8, 1, 1, np.array([0.0, 0.1], np.float32)), (0, 1, 1, temps)]:
         with pytest.raises(hsg.HsgError):
             hsg.hsg_query_bytes(*bad)
+    # hsg_desc.flags: the fast-math heat-bath variant is the only defined bit; unknown bits are refused
+    assert hsg.hsg_query_bytes(8, 2, 2, temps, flags=hsg.HSG_FLAG_FAST_MATH) == (state, scratch)
+    for flags in (2, 4, 0x80000000, 3):
+        with pytest.raises(hsg.HsgError):
+            hsg.hsg_query_bytes(8, 2, 2, temps, flags=flags)
+    text = (ROOT / "include" / "hsg.h").read_text()
+    assert re.search(r"HSG_FLAG_FAST_MATH\s*=\s*1\b", text) and hsg.HSG_FLAG_FAST_MATH == 1
 
 
 def test_null_handles_are_rejected():

@@ -63,15 +63,21 @@ void dm_or_reflect(long n, const float* s, const float* h, float* o, int packed)
     o[3*j] = f2_hi(r.x); o[3*j+1] = f2_hi(r.y); o[3*j+2] = f2_hi(r.z);
   }
 }
-void dm_hb_draw(long n, const float* h, const float* beta, const float* u1, const float* u2, float* o, int packed) {
+// variant: 0 = the reference draw hb_draw, 1 = hb_draw_fast (HSG_FLAG_FAST_MATH)
+void dm_hb_draw(long n, const float* h, const float* beta, const float* u1, const float* u2, float* o, int packed, int variant) {
   if (!packed) {
-    for (long i = 0; i < n; ++i) { const Vec3 r = hb_draw(Vec3{h[3*i], h[3*i+1], h[3*i+2]}, beta[i], u1[i], u2[i]); o[3*i] = r.x; o[3*i+1] = r.y; o[3*i+2] = r.z; }
+    for (long i = 0; i < n; ++i) {
+      const Vec3 hv = {h[3*i], h[3*i+1], h[3*i+2]};
+      const Vec3 r = variant ? hb_draw_fast(hv, beta[i], u1[i], u2[i]) : hb_draw(hv, beta[i], u1[i], u2[i]);
+      o[3*i] = r.x; o[3*i+1] = r.y; o[3*i+2] = r.z;
+    }
     return;
   }
   for (long i = 0; i + 1 < n; i += 2) {     // the two sites of a pair share beta (one system): beta[i]
     const long j = i + 1;
     const V3<F2> hv = {make_f2(h[3*i], h[3*j]), make_f2(h[3*i+1], h[3*j+1]), make_f2(h[3*i+2], h[3*j+2])};
-    const V3<F2> r = hb_draw(hv, beta[i], make_f2(u1[i], u1[j]), make_f2(u2[i], u2[j]));
+    const F2 a1 = make_f2(u1[i], u1[j]), a2 = make_f2(u2[i], u2[j]);
+    const V3<F2> r = variant ? hb_draw_fast(hv, beta[i], a1, a2) : hb_draw(hv, beta[i], a1, a2);
     o[3*i] = f2_lo(r.x); o[3*i+1] = f2_lo(r.y); o[3*i+2] = f2_lo(r.z);
     o[3*j] = f2_hi(r.x); o[3*j+1] = f2_hi(r.y); o[3*j+2] = f2_hi(r.z);
   }
@@ -104,7 +110,7 @@ def dm(tmp_path_factory):
     L.dm_sqrt.argtypes = [lg, vp, vp, i32]
     L.dm_series.argtypes = [lg, vp, vp, vp, vp, vp]
     L.dm_or_reflect.argtypes = [lg, vp, vp, vp, i32]
-    L.dm_hb_draw.argtypes = [lg, vp, vp, vp, vp, vp, i32]
+    L.dm_hb_draw.argtypes = [lg, vp, vp, vp, vp, vp, i32, i32]
     return L
 
 
@@ -235,10 +241,52 @@ def test_heat_bath_agrees_with_the_oracle_bit_for_bit(dm, packed):
     u1[:8] = [2.0**-24, 1 - 2.0**-24, 0.5, 0.25, 2.0**-24, 1 - 2.0**-24, 0.75, 0.5]
     u2[:8] = [2.0**-24, 1 - 2.0**-24, 0.125, 0.375, 0.625, 0.875, 0.25, 0.5]
     o = np.zeros((n, 3), dtype=np.float32)
-    dm.dm_hb_draw(n, _p(h), _p(beta), _p(u1), _p(u2), _p(o), packed)
+    dm.dm_hb_draw(n, _p(h), _p(beta), _p(u1), _p(u2), _p(o), packed, 0)
     ref = np.array([oracle.hb_draw(h[i], beta[i], u1[i], u2[i], precision=32) for i in range(n)], dtype=np.float32)
     a = beta.astype(np.float64) * hn
     assert (a == 0).any() and ((a > 0) & (a < 1e-4)).any() and ((a > 1e-4) & (a < 0.05)).any() and (a > 50).any()
     bad = np.nonzero((_bits(o) != _bits(ref)).any(axis=1))[0]
     assert len(bad) == 0, (len(bad), bad[:5], a[bad[:5]], o[bad[:5]], ref[bad[:5]])
     assert np.abs(np.linalg.norm(o.astype(np.float64), axis=1) - 1).max() < 1e-5
+
+
+def fast_math_bound(a):
+    """Stated parity bound of the fast-math heat-bath variant (include/hsg.h HSG_FLAG_FAST_MATH): per
+    component, one update from equal inputs.  t = 1 - cos(theta) carries an absolute error eps_t ~ 2^-21 (1 + 1/a) (the
+    special-function unit's 2^-22 bounds on e^{-2a}, lg2 and 1/a, and the rounding of 1 - y before the logarithm, divided
+    by a); sin(theta) = sqrt(t (2 - t)) turns it into up to sqrt(2 eps_t) for draws next to the poles."""
+    return np.sqrt(2e-6 * (1.0 + 1.0 / a))
+
+
+@pytest.mark.parametrize("packed", [0, 1])
+@pytest.mark.parametrize("jitter", [0, 2])
+def test_fast_math_heat_bath_variant_stays_inside_its_stated_bound(dm, packed, jitter):
+    """hb_draw_fast against the reference draw on the same (h, beta, u1, u2): the host model of the special-function unit is
+    libm (jitter 0) or libm plus errors of the full size the PTX ISA allows (jitter 2).  Every draw inside the stated
+    bound, the typical draw far inside it, unit norm kept, and the series branch (a < 1e-4) unchanged bit for bit."""
+    dm.dm_set_jitter(jitter)
+    rng = np.random.default_rng(7)
+    n = 400_000
+    h = (rng.normal(size=(n, 3)) * np.exp(rng.uniform(-9, 2, (n, 1)))).astype(np.float32)
+    h[::977] = 0.0
+    beta = np.exp(rng.uniform(np.log(1e-6), np.log(30.0), n)).astype(np.float32)
+    beta[1::2] = beta[::2]
+    u1 = ((rng.integers(0, 2**23, n).astype(np.float64) + 0.5) * 2.0**-23).astype(np.float32)
+    u2 = ((rng.integers(0, 2**23, n).astype(np.float64) + 0.5) * 2.0**-23).astype(np.float32)
+    ref = np.zeros((n, 3), dtype=np.float32); o = np.zeros((n, 3), dtype=np.float32)
+    dm.dm_hb_draw(n, _p(h), _p(beta), _p(u1), _p(u2), _p(ref), 0, 0)
+    dm.dm_hb_draw(n, _p(h), _p(beta), _p(u1), _p(u2), _p(o), packed, 1)
+    dm.dm_set_jitter(2)
+    assert np.isfinite(o).all()
+    a = beta.astype(np.float64) * np.linalg.norm(h.astype(np.float64), axis=1)
+    dev = np.abs(o.astype(np.float64) - ref.astype(np.float64)).max(axis=1)
+    big = a >= 1e-4
+    assert (dev[big] <= fast_math_bound(a[big])).all(), (dev[big] / fast_math_bound(a[big])).max()
+    assert np.median(dev[big] / (1.0 + 1.0 / a[big])) < 1e-6
+    # below the switch the draw is the series of the reference arithmetic; only 1/|h| and the azimuth are approximated
+    small = (a < 1e-4)
+    assert small.any() and dev[small].max() < 4e-6
+    assert np.abs(np.linalg.norm(o.astype(np.float64), axis=1) - 1).max() < 1e-5
+    for lo, hi in ((1, 10), (10, 1e3)):                      # BASELINE.json's ladders live here: a = |h|/T with T <= 0.3
+        m = (a >= lo) & (a < hi)
+        assert np.quantile(dev[m], 0.999) < 1e-5
