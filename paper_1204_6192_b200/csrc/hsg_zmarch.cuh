@@ -201,6 +201,7 @@ template <int L, int YS, int V, int G> struct Cfg {
   static_assert(!HALO || V == 4, "halo copies use 16-byte cp.async.cg");
   static_assert(!HALO || YS >= 2, "a thread is on at most one strip edge");
   static_assert(NJB <= 6, "mbarrier area holds NJB J/H barriers and two halo barriers");
+  static_assert(!HALO || DJ >= 2, "strip kernels: J/H ring depth 1 faulted at L = 64, G = 1 (round 1) and its cause is not established; only DJ >= 2 is validated");
   static constexpr uint32_t halo_bytes = G * 2u * 3u * Lh * 4u;   // new colour-0 halo rows received per step: both neighbours, G systems
   static_assert(smem_bytes <= 232448, "exceeds the 227 KB of shared memory per CTA");
 };

@@ -30,7 +30,9 @@ def shard_bounds(n_samples: int, world_size: int) -> List[Tuple[int, int]]:
 
 
 def shard_of_rank(n_samples: int, world_size: int, rank: int) -> Tuple[int, int]:
-    """(sample_offset, count) of ``rank``: pass them to ``hsg_create(..., n_samples=count, sample_offset=offset)``."""
+    """(sample_offset, count) of ``rank``: pass them to ``hsg_create(..., n_samples=count, sample_offset=offset)``.
+    count == 0 (more ranks than samples): the rank creates no engine (``hsg_create`` refuses an empty context) and passes a
+    zero-length tensor to ``gather_by_sample``."""
     if not 0 <= rank < world_size:
         raise ValueError("shard_of_rank: rank out of range")
     return shard_bounds(n_samples, world_size)[rank]
