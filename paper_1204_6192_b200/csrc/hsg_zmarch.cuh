@@ -695,7 +695,7 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
 #pragma unroll
-      for (int o = RW / 2; o > 0; o >>= 1) v[i] += __shfl_down_sync(0xffffffffu, v[i], o, RW);
+      for (int o = RW / 2; o > 0; o >>= 1) v[i] += __shfl_down_sync(th.lanes, v[i], o, RW);   // (th.lanes: a 16-thread CTA has half a warp)
     }
     if (tl % RW == 0) {
 #pragma unroll
@@ -773,14 +773,17 @@ inline cudaError_t zmarch_launch_g(const ZmarchArgs& a, cudaStream_t stream, int
   return zmarch_launch_t<L, T::YS, T::V, G>(a, stream);
 }
 
-// Systems per CTA: the G slots of a CTA must belong to one sample (G divides O*T); G shrinks (down to 1) while the grid
-// would leave at least half of the SMs without a CTA.  (Measured on the paper's Table-1 workload, 256 systems of L = 32:
+// Systems per CTA: the G slots of a CTA must belong to one sample (G divides O*T); G shrinks while the grid would leave at
+// least half of the SMs without a CTA, but not below one full warp per CTA where divisibility allows (L = 8: 16 threads per system).  (Measured on the paper's Table-1 workload, 256 systems of L = 32:
 // 128 CTAs of G = 2 run 6.1 ps/update, 256 CTAs of G = 1 run 8.0 — a second wave costs more than 20 idle SMs.)
 template <int L>
 inline int zmarch_pick_g(const Geom& g, int sm_count) {
-  int G = zm::Tune<L>::GMAX;
+  using T = zm::Tune<L>;
+  // threads of one system in the launch with the fewest threads per system (V >= VHB): a CTA keeps at least one full warp
+  constexpr int TPS_MIN = T::YS * (L / 2 / T::V);
+  int G = T::GMAX;
   while (G > 1 && (g.O * g.T) % G != 0) G >>= 1;
-  while (G > 1 && 2 * (long long)(g.R / G) * (L / zm::Tune<L>::YS) <= sm_count) G >>= 1;
+  while (G > 1 && (G / 2) * TPS_MIN >= 32 && 2 * (long long)(g.R / G) * (L / T::YS) <= sm_count) G >>= 1;
   return G;
 }
 
