@@ -38,6 +38,7 @@
 #include "hsg_layout.cuh"
 #include "hsg_math.cuh"
 #include "hsg_zmarch_launch.h"
+#include "hsg_zmarch_ptx.cuh"
 
 namespace hsg {
 
@@ -57,111 +58,6 @@ template <> struct Tune<32> { static constexpr int YS = 32, V = 4, VHB = 2, GMAX
 template <> struct Tune<64> { static constexpr int YS = 16, V = 4, VHB = 4, GMAX = 2, DS = 2, DJ = 2; };
 constexpr int kUnroll = 2;     // unroll factor of the main march loop (over-relaxation / heat bath)
 constexpr int kUnrollHB = 2;
-
-// ---------------------------------------------------------------- PTX wrappers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ uint64_t policy_evict_first() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ uint64_t policy_evict_last() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-// per-thread async copy of 4V bytes global -> shared (streaming: evict-first in L2)
-template <int V> __device__ __forceinline__ void cp_async(uint32_t dst, const float* src, uint64_t pol);
-template <> __device__ __forceinline__ void cp_async<2>(uint32_t dst, const float* src, uint64_t pol) {
-  asm volatile("cp.async.ca.shared.global.L2::cache_hint [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "l"(pol) : "memory");
-}
-template <> __device__ __forceinline__ void cp_async<4>(uint32_t dst, const float* src, uint64_t pol) {
-  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-// thread-block cluster helpers (strips of one lattice, see the header comment)
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-  return r;
-}
-__device__ __forceinline__ uint32_t mapa_u32(uint32_t cta_addr, uint32_t rank) {
-  uint32_t r;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(cta_addr), "r"(rank));
-  return r;
-}
-__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
-__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
-__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
-__device__ __forceinline__ void st_cluster_f64(uint32_t addr, double v) {
-  asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
-}
-
-// ---------------------------------------------------------------- V-wide vector access: V = 2 or 4 floats = V/2 packed pairs
-// (hsg_math.cuh: F2 = two binary32 lanes in an aligned register pair; lane e&1 of pair e>>1 is compact site j0 + e)
-
-// shared memory by 32-bit shared-window byte address (keeps all address arithmetic 32-bit)
-template <int V> __device__ __forceinline__ void lds(F2 (&r)[V / 2], uint32_t a);
-template <> __device__ __forceinline__ void lds<2>(F2 (&r)[1], uint32_t a) {
-  asm volatile("ld.shared.b64 %0, [%1];" : "=l"(r[0].v) : "r"(a) : "memory");
-}
-template <> __device__ __forceinline__ void lds<4>(F2 (&r)[2], uint32_t a) {
-  asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(r[0].v), "=l"(r[1].v) : "r"(a) : "memory");
-}
-template <int V> __device__ __forceinline__ void sts(uint32_t a, const F2 (&r)[V / 2]);
-template <> __device__ __forceinline__ void sts<2>(uint32_t a, const F2 (&r)[1]) {
-  asm volatile("st.shared.b64 [%0], %1;" ::"r"(a), "l"(r[0].v) : "memory");
-}
-template <> __device__ __forceinline__ void sts<4>(uint32_t a, const F2 (&r)[2]) {
-  asm volatile("st.shared.v2.b64 [%0], {%1,%2};" ::"r"(a), "l"(r[0].v), "l"(r[1].v) : "memory");
-}
-// asynchronous store into the shared memory of another CTA of the cluster (addresses from mapa_u32); the bytes are
-// counted on an mbarrier of THAT CTA, whose threads wait on it: no fence on either side
-template <int V> __device__ __forceinline__ void st_async(uint32_t a, const F2 (&r)[V / 2], uint32_t bar);
-template <> __device__ __forceinline__ void st_async<2>(uint32_t a, const F2 (&r)[1], uint32_t bar) {
-  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];"
-               ::"r"(a), "l"(r[0].v), "r"(bar) : "memory");
-}
-template <> __device__ __forceinline__ void st_async<4>(uint32_t a, const F2 (&r)[2], uint32_t bar) {
-  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1,%2}, [%3];"
-               ::"r"(a), "l"(r[0].v), "l"(r[1].v), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-// streaming global access for the spins: each value is touched once per sweep
-template <int V> __device__ __forceinline__ void ldg(F2 (&r)[V / 2], const float* p);
-template <> __device__ __forceinline__ void ldg<2>(F2 (&r)[1], const float* p) {
-  const float2 t = __ldcs(reinterpret_cast<const float2*>(p));
-  r[0] = make_f2(t.x, t.y);
-}
-template <> __device__ __forceinline__ void ldg<4>(F2 (&r)[2], const float* p) {
-  const float4 t = __ldcs(reinterpret_cast<const float4*>(p));
-  r[0] = make_f2(t.x, t.y); r[1] = make_f2(t.z, t.w);
-}
-template <int V> __device__ __forceinline__ void stg(float* p, const F2 (&r)[V / 2]);
-template <> __device__ __forceinline__ void stg<2>(float* p, const F2 (&r)[1]) {
-  __stcs(reinterpret_cast<float2*>(p), make_float2(f2_lo(r[0]), f2_hi(r[0])));
-}
-template <> __device__ __forceinline__ void stg<4>(float* p, const F2 (&r)[2]) {
-  __stcs(reinterpret_cast<float4*>(p), make_float4(f2_lo(r[0]), f2_hi(r[0]), f2_lo(r[1]), f2_hi(r[1])));
-}
 
 template <int L, int YS, int V, int G> struct Cfg {
   static constexpr int Lh = L / 2;
@@ -273,7 +169,7 @@ __device__ __forceinline__ void update_sites(F2 (&out)[3][V / 2], const F2 (&own
     F2 t[NP];
     lds<V>(t, ja.oth_xy + th.row0);
     // the bond from x-1 is the +x coupling stored at the other colour's site j-1+off: the thread's own t[] when off = 1
-    const float te = __shfl_sync(th.lanes, f2_hi(t[NP - 1]), th.lane_prev);
+    const float te = shfl_idx(th.lanes, f2_hi(t[NP - 1]), th.lane_prev);
 #pragma unroll
     for (int p = 0; p < NP; ++p) Jxm[p] = up ? t[p] : shifted(t, te, p);
   }
@@ -287,7 +183,7 @@ __device__ __forceinline__ void update_sites(F2 (&out)[3][V / 2], const F2 (&own
     lds<V>(Hm, ja.own_h + mu * CJB + th.row0);
     lds<V>(yp, xs_p + mu * CSB);
     lds<V>(ym, xs_m + mu * CSB);
-    const float se = __shfl_sync(th.lanes, up ? f2_lo(q[mu][0]) : f2_hi(q[mu][NP - 1]), src);
+    const float se = shfl_idx(th.lanes, up ? f2_lo(q[mu][0]) : f2_hi(q[mu][NP - 1]), src);
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
       const F2 sh = shifted(q[mu], se, p);
@@ -356,8 +252,8 @@ __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __res
   // copies of a plane are issued by the first lanes of different warps (two for a whole plane, four for a strip)
   constexpr bool TWO = !C::HALO && C::NT > 32;
   constexpr bool FOUR = C::HALO && C::NT >= 128;
-  if (FOUR ? ((threadIdx.x & 31u) == 0 && threadIdx.x < 128) : (threadIdx.x < 32 || (TWO && threadIdx.x == 32))) {
-    const int upto = min(nd + C::DJ, st.total - 1);
+  if (FOUR ? ((tid_x() & 31u) == 0 && tid_x() < 128) : (tid_x() < 32 || (TWO && tid_x() == 32))) {
+    const int upto = imin(nd + C::DJ, st.total - 1);
     while (st.issued < upto) {
       ++st.issued;
       const int plane = (st.issued + L - 1) % L;
@@ -365,22 +261,20 @@ __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __res
       const uint32_t dA = sm.ja + ((uint32_t)st.issued % C::NJA) * JAB, dB = sm.jb + ((uint32_t)st.issued % C::NJB) * JBB;
       const float* src = jh_d + (size_t)plane * 12 * C::CSG;
       if (!C::HALO) {
-        if (threadIdx.x == 0) {
-          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(JAB + JBB) : "memory");
-          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                       ::"r"(dA), "l"(src), "r"(JAB), "r"(bar), "l"(pol) : "memory");
+        if (tid_x() == 0) {
+          mbar_expect_tx(bar, JAB + JBB);
+          bulk_g2s(dA, src, JAB, bar, pol);
         }
-        if (threadIdx.x == (TWO ? 32 : 0))     // (its complete_tx may land before the expect_tx: the phase still needs that arrive)
-          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                       ::"r"(dB), "l"(src + 11 * C::CSG), "r"(JBB), "r"(bar), "l"(pol) : "memory");
+        if (tid_x() == (TWO ? 32 : 0))     // (its complete_tx may land before the expect_tx: the phase still needs that arrive)
+          bulk_g2s(dB, src + 11 * C::CSG, JBB, bar, pol);
       } else {
         // strip-major J/H layout (hsg_layout.cuh): the twelve arrays of this strip of the plane are contiguous; the row
         // y0-1 of the two Jy arrays comes from the last row of the strip below.  Four copies, one per lane.
         constexpr uint32_t ROWB = 4u * C::Lh, STRIPB = 4u * C::YSv * C::Lh;
-        const int lane = FOUR ? (int)(threadIdx.x >> 5) : (int)threadIdx.x;      // which of the four copies
+        const int lane = FOUR ? (int)(tid_x() >> 5) : (int)tid_x();      // which of the four copies
         if (lane == 0)       // (a complete_tx that lands before this expect_tx is fine: the phase still needs the arrive)
-          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(12u * STRIPB + 2u * ROWB) : "memory");
-        if (!FOUR) __syncwarp();
+          mbar_expect_tx(bar, 12u * STRIPB + 2u * ROWB);
+        if (!FOUR) warp_sync();
         if (lane < 4) {
           const int strip = sm.y0 / C::YSv, below = (strip + C::NCL - 1) % C::NCL;
           const float* blk = src + (size_t)strip * 12 * C::CSJ;
@@ -388,8 +282,7 @@ __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __res
           const uint32_t dst = lane == 0 ? dA : lane == 1 ? dB : dA + 11u * JBB + (uint32_t)(lane - 2) * ROWB;
           const float* from = lane == 0 ? blk : lane == 1 ? blk + 11 * C::CSJ : blo + (lane == 2 ? 1 : 6) * C::CSJ;
           const uint32_t bytes = lane == 0 ? 11u * STRIPB : lane == 1 ? STRIPB : ROWB;
-          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
-                       ::"r"(dst), "l"(from), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+          bulk_g2s(dst, from, bytes, bar, pol);
         }
       }
     }
@@ -398,15 +291,7 @@ __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __res
     ++st.waited;
     const uint32_t bar = sm.full + 8u * ((uint32_t)st.waited % C::NJB);
     const uint32_t parity = ((uint32_t)st.waited / C::NJB) & 1u;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
+    mbar_wait(bar, parity);
   }
 }
 
@@ -421,7 +306,7 @@ __device__ __forceinline__ void ring_advance(const SmemT& sm, const float* __res
 // (st.async complete_tx).  Only the last arrive of a sweep RELEASES, pairing with the acquiring wait of the next
 // prologue: it makes the new colour-1 rows in global memory visible to the neighbour that fetches them as halo rows.
 template <class C, bool RELEASE = false> __device__ __forceinline__ void step_end() {
-  __syncthreads();
+  cta_sync();
   if (C::HALO) { if (RELEASE) cluster_arrive(); else cluster_arrive_relaxed(); }
 }
 template <class C> __device__ __forceinline__ void step_wait() {
@@ -477,7 +362,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   // the previous step), every thread waits for the bytes before the colour-1 update that reads them; bit `par` of hph
   // is the parity of the phase in flight
   auto arm_halo = [&](uint32_t par) {
-    if (HALO && threadIdx.x == 0) mbar_expect_tx(sm.hfull + 8u * par, C::halo_bytes);
+    if (HALO && tid_x() == 0) mbar_expect_tx(sm.hfull + 8u * par, C::halo_bytes);
   };
   auto wait_halo = [&](uint32_t par) {
     if (HALO) { mbar_wait(sm.hfull + 8u * par, (hph >> par) & 1u); hph ^= 1u << par; }
@@ -588,11 +473,11 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
 template <int L, int YS, int V, int G, bool FM>
 __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchArgs a) {
   using C = Cfg<L, YS, V, G>;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
+  HSG_DYN_SMEM(smem_raw);
   const uint32_t base = smem_u32(smem_raw);
-  const int gs = threadIdx.x / C::TPS, tl = threadIdx.x % C::TPS;
+  const int gs = tid_x() / C::TPS, tl = tid_x() % C::TPS;
   const int rank = C::HALO ? (int)cluster_ctarank() : 0;   // strip index
-  const int group = C::HALO ? (int)(blockIdx.x / C::NCL) : (int)blockIdx.x;
+  const int group = C::HALO ? (int)(ctaid_x() / C::NCL) : (int)ctaid_x();
   Smem sm;
   sm.full = base;
   sm.hfull = base + 48;
@@ -602,12 +487,12 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
   sm.x0 = sm.c1 + 4u * C::NC1 * C::HPS;
   sm.c0 = sm.x0 + 4u * 2 * C::HPS;
   sm.y0 = rank * YS;
-  if (threadIdx.x == 0) {
+  if (tid_x() == 0) {
 #pragma unroll
     for (int i = 0; i < C::NJB; ++i) mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + i, 1);
     mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + 6, 1);
     mbar_init(reinterpret_cast<uint64_t*>(smem_raw) + 7, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_mbarrier_init();
   }
   step_end<C, true>();                                   // strips: the first wait (in the prologue) sees every CTA of the cluster running
 
@@ -646,7 +531,7 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
     // the TPR threads of a row are consecutive lanes of one warp (TPR divides 32)
     static_assert(32 % C::TPR == 0 || C::TPR % 32 == 0, "a row occupies whole warps or a power-of-two part of one");
     static_assert(C::TPR <= 32, "a row must fit one warp: its x neighbours travel by shuffle");
-    const int lane = (int)(threadIdx.x & 31u), first = lane & ~(C::TPR - 1);
+    const int lane = (int)(tid_x() & 31u), first = lane & ~(C::TPR - 1);
     th.lane_prev = first | ((lane - 1) & (C::TPR - 1));
     th.lane_next = first | ((lane + 1) & (C::TPR - 1));
     th.lanes = C::NT >= 32 ? 0xffffffffu : ((1u << (C::NT & 31)) - 1u);
@@ -695,13 +580,13 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
 #pragma unroll
-      for (int o = RW / 2; o > 0; o >>= 1) v[i] += __shfl_down_sync(th.lanes, v[i], o, RW);   // (th.lanes: a 16-thread CTA has half a warp)
+      for (int o = RW / 2; o > 0; o >>= 1) v[i] += shfl_down(th.lanes, v[i], o, RW);   // (th.lanes: a 16-thread CTA has half a warp)
     }
     if (tl % RW == 0) {
 #pragma unroll
       for (int i = 0; i < 4; ++i) red[(gs * WPS + tl / RW) * 4 + i] = v[i];
     }
-    __syncthreads();
+    cta_sync();
     double x = 0.0;
     if (tl < 4)
       for (int w = 0; w < WPS; ++w) x += red[(gs * WPS + w) * 4 + tl];
@@ -723,83 +608,5 @@ __global__ void __launch_bounds__(Cfg<L, YS, V, G>::NT, 1) zmarch_kernel(ZmarchA
 }
 
 }  // namespace zm
-
-// ------------------------------------------------------------------------------------------------ host side
-template <int L, int YS, int V, int G, bool FM = false>
-inline cudaError_t zmarch_launch_t(const ZmarchArgs& a, cudaStream_t stream) {
-  using C = zm::Cfg<L, YS, V, G>;
-  // the attribute is per device: set it on every launch (a host-side table lookup) rather than remember per process,
-  // so that contexts on several devices of one process work (hsg.h: "distinct contexts are independent")
-  const cudaError_t e = cudaFuncSetAttribute(zm::zmarch_kernel<L, YS, V, G, FM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::smem_bytes);
-  if (e != cudaSuccess) return e;
-  if (C::NCL == 1) {
-    zm::zmarch_kernel<L, YS, V, G, FM><<<a.g.R / G, C::NT, C::smem_bytes, stream>>>(a);
-    return cudaGetLastError();
-  }
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)(a.g.R / G * C::NCL));
-  cfg.blockDim = dim3(C::NT);
-  cfg.dynamicSmemBytes = C::smem_bytes;
-  cfg.stream = stream;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = C::NCL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, zm::zmarch_kernel<L, YS, V, G, FM>, a);
-}
-
-// hsg_sweep(n_or, n_hb) at lattice size L with G systems per CTA: one launch, or (VHB != V and both phases present) an
-// over-relaxation launch followed by a heat-bath launch; E and m are reduced by whichever launch holds the final sweep
-template <int L, int G>
-inline cudaError_t zmarch_launch_g(const ZmarchArgs& a, cudaStream_t stream, int* n_launch) {
-  using T = zm::Tune<L>;
-  *n_launch = 1;
-  if (T::VHB != T::V && a.n_hb > 0) {
-    if (a.n_or > 0) {
-      ZmarchArgs o = a;
-      o.n_hb = 0; o.e_slot = nullptr;
-      const cudaError_t e = zmarch_launch_t<L, T::YS, T::V, G>(o, stream);
-      if (e != cudaSuccess) return e;
-      *n_launch = 2;
-    }
-    ZmarchArgs h = a;
-    h.n_or = 0;
-    return a.fast_math ? zmarch_launch_t<L, T::YS, T::VHB, G, true>(h, stream) : zmarch_launch_t<L, T::YS, T::VHB, G>(h, stream);
-  }
-  // (only a launch that holds heat-bath sweeps has a fast-math form: over-relaxation is the reference arithmetic either way)
-  if constexpr (T::VHB == T::V) {
-    if (a.fast_math && a.n_hb > 0) return zmarch_launch_t<L, T::YS, T::V, G, true>(a, stream);
-  }
-  return zmarch_launch_t<L, T::YS, T::V, G>(a, stream);
-}
-
-// Systems per CTA: the G slots of a CTA must belong to one sample (G divides O*T); G shrinks while the grid would leave at
-// least half of the SMs without a CTA, but not below one full warp per CTA where divisibility allows (L = 8: 16 threads per system).  (Measured on the paper's Table-1 workload, 256 systems of L = 32:
-// 128 CTAs of G = 2 run 6.1 ps/update, 256 CTAs of G = 1 run 8.0 — a second wave costs more than 20 idle SMs.)
-template <int L>
-inline int zmarch_pick_g(const Geom& g, int sm_count) {
-  using T = zm::Tune<L>;
-  // threads of one system in the launch with the fewest threads per system (V >= VHB): a CTA keeps at least one full warp
-  constexpr int TPS_MIN = T::YS * (L / 2 / T::V);
-  int G = T::GMAX;
-  while (G > 1 && (g.O * g.T) % G != 0) G >>= 1;
-  while (G > 1 && (G / 2) * TPS_MIN >= 32 && 2 * (long long)(g.R / G) * (L / T::YS) <= sm_count) G >>= 1;
-  return G;
-}
-
-template <int L, int G>
-inline cudaError_t zmarch_dispatch_g(const ZmarchArgs& a, cudaStream_t stream, int* n_launch, int want_g) {
-  if (want_g == G) return zmarch_launch_g<L, G>(a, stream, n_launch);
-  if constexpr (G > 1) return zmarch_dispatch_g<L, G / 2>(a, stream, n_launch, want_g);
-  *n_launch = 0;
-  return cudaErrorNotSupported;
-}
-
-// body of the per-size entry points zmarch_launch_l<L> (hsg_zmarch_l8.cu ... hsg_zmarch_l64.cu: one translation unit per
-// lattice size, compiled in parallel)
-template <int L>
-inline cudaError_t zmarch_launch_size(const ZmarchArgs& a, cudaStream_t stream, int* n_launch, int sm_count) {
-  return zmarch_dispatch_g<L, zm::Tune<L>::GMAX>(a, stream, n_launch, zmarch_pick_g<L>(a.g, sm_count));
-}
 
 }  // namespace hsg

@@ -1,5 +1,5 @@
 // hsg_zmarch_l16.cu — instantiations of the z-marching sweep kernel for L = 16 (hsg_zmarch.cuh, Tune<16>).
-#include "hsg_zmarch.cuh"
+#include "hsg_zmarch_dispatch.cuh"
 
 namespace hsg {
 cudaError_t zmarch_launch_l16(const ZmarchArgs& a, cudaStream_t stream, int* n_launch, int sm_count) {

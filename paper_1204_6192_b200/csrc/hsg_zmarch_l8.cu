@@ -1,5 +1,5 @@
 // hsg_zmarch_l8.cu — instantiations of the z-marching sweep kernel for L = 8 (hsg_zmarch.cuh, Tune<8>).
-#include "hsg_zmarch.cuh"
+#include "hsg_zmarch_dispatch.cuh"
 
 namespace hsg {
 cudaError_t zmarch_launch_l8(const ZmarchArgs& a, cudaStream_t stream, int* n_launch, int sm_count) {
