@@ -378,7 +378,7 @@ __device__ __forceinline__ void march_sweep(const Smem& sm, float* __restrict__ 
   for (int mu = 0; mu < 3; ++mu) {
     ldg<V>(A[mu], Sr + (L - 1) * PS + HP + mu * CS);
 #pragma unroll
-    for (int e = 0; e < NP; ++e) { P[mu][e].v = 0ull; Q[mu][e].v = 0ull; O[mu][e].v = 0ull; On[mu][e].v = 0ull; }
+    for (int e = 0; e < NP; ++e) { P[mu][e] = make_f2(0.0f, 0.0f); Q[mu][e] = P[mu][e]; O[mu][e] = P[mu][e]; On[mu][e] = P[mu][e]; }
   }
   cp_async_wait<C::DS>();
 #pragma unroll

@@ -17,3 +17,10 @@ static inline float __fadd_rn(float a, float b) { return a + b; }
 static inline float __fsub_rn(float a, float b) { return a - b; }
 static inline float __uint_as_float(uint32_t w) { float f; std::memcpy(&f, &w, 4); return f; }
 static inline uint32_t __float_as_uint(float f) { uint32_t w; std::memcpy(&w, &f, 4); return w; }
+
+// kernel qualifiers and the handful of runtime types the kernel headers mention (tests/test_zmarch_on_host.py)
+#define __global__
+#define __launch_bounds__(...)
+typedef int cudaError_t;
+typedef void* cudaStream_t;
+enum { cudaSuccess = 0, cudaErrorNotSupported = 801 };
