@@ -13,6 +13,7 @@
 
 #include "hsg_kernels.cuh"
 #include "hsg_observables.cuh"
+#include "hsg_shapes.h"
 #include "hsg_zmarch_launch.h"
 
 using namespace hsg;
@@ -85,7 +86,6 @@ Geom make_geom(const hsg_desc* d) {
   return g;
 }
 
-inline unsigned blocks_for(long long n) { return (unsigned)((n + kThreads - 1) / kThreads); }
 
 }  // namespace
 
@@ -300,25 +300,6 @@ int hsg_sweep(hsg_ctx* ctx, int n_or, int n_hb) {
 }
 
 // ------------------------------------------------------------------ energy, parallel tempering, measurements
-// planes per block of the reduction kernels: about 4 vector items per thread, at most L chunks per system
-static int reduce_zb(const Geom& g, int V) {
-  const int ipp = 2 * g.L * (g.Lh / V);
-  int zb = (4 * kThreads + ipp - 1) / ipp;
-  if (zb < 1) zb = 1;
-  if (zb > g.L) zb = g.L;
-  return zb;
-}
-static int vec_width(const Geom& g) { return (g.Lh % 4 == 0) ? 4 : (g.Lh % 2 == 0) ? 2 : 1; }
-
-// a block takes a chunk of planes of one (sample[, pair], temperature): whole lattices up to L = 32, 16 planes beyond
-static void reduction_shape(const Geom& g, int V, int* ZB, int* n_chunks, int* nt) {
-  *ZB = g.L > 32 ? 16 : g.L;
-  *n_chunks = (g.L + *ZB - 1) / *ZB;
-  int n = 32;
-  while (n < kThreads && ((long long)*ZB * g.L * (g.Lh / V) >= 8LL * n || n < 2 * (g.Lh / V))) n *= 2;
-  *nt = n;
-}
-
 static int enqueue_energy_mag(hsg_ctx* ctx) {
   const Geom& g = ctx->g;
   if (ctx->energy_valid) return HSG_OK;          // spins unchanged since the last reduction

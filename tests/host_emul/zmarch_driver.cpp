@@ -92,6 +92,7 @@ extern "C" int EMU_CAT(emu_zmarch_l, EMU_L)(int G, int mode, int D, int O, int T
   ZmarchArgs a{g, priv.data(), jh.data(), temp_of_slot.data(), beta.data(), PhiloxKey{(uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)},
                k_hb, n_or, n_hb, E ? e_slot.data() : nullptr, m_slot.data(), 0};
   emu::mode = mode;
+  hsg::seed_jitter = 0;      // exact reciprocal seeds (the variable is shared with any other host build loaded in this process)
   const int rc = dispatch<L>(G, a);
   if (rc != 0) return rc;
   convert(false);
