@@ -9,7 +9,7 @@ using namespace hsg;
 
 namespace {
 
-template <int L, int YS, int V, int G>
+template <int L, int YS, int V, int G, bool FM = false>
 void launch(const ZmarchArgs& a) {
   using C = zm::Cfg<L, YS, V, G>;
   std::vector<uint32_t> mbars;
@@ -17,7 +17,7 @@ void launch(const ZmarchArgs& a) {
   const int n_groups = a.g.R / G;
   for (int grp = 0; grp < n_groups; ++grp) {                          // one cluster (or CTA) after the other
     emu::Launch ln(C::NCL, C::NT, C::smem_bytes, (unsigned)(grp * C::NCL), mbars);
-    ln.run([&a] { zm::zmarch_kernel<L, YS, V, G, false>(a); });
+    ln.run([&a] { zm::zmarch_kernel<L, YS, V, G, FM>(a); });
   }
 }
 
@@ -28,8 +28,11 @@ void sweep(const ZmarchArgs& a) {
   if (T::VHB != T::V && a.n_hb > 0) {
     if (a.n_or > 0) { ZmarchArgs o = a; o.n_hb = 0; o.e_slot = nullptr; launch<L, T::YS, T::V, G>(o); }
     ZmarchArgs h = a; h.n_or = 0;
-    launch<L, T::YS, T::VHB, G>(h);
+    if (a.fast_math) launch<L, T::YS, T::VHB, G, true>(h); else launch<L, T::YS, T::VHB, G>(h);
     return;
+  }
+  if constexpr (T::VHB == T::V) {
+    if (a.fast_math && a.n_hb > 0) { launch<L, T::YS, T::V, G, true>(a); return; }
   }
   launch<L, T::YS, T::V, G>(a);
 }
@@ -52,10 +55,10 @@ int dispatch(int G, const ZmarchArgs& a) {
 #define EMU_CAT(a, b) EMU_CAT2(a, b)
 
 // S: canonical spins [D][O][T][3][N] (configuration t of a chain holds temperature t), updated in place;
-// E [R], M [R][3]: the fused reductions of the final sweep.  mode: 0 = asynchronous copies land when issued, 1 = when waited for.
+// E [R], M [R][3]: the fused reductions of the final sweep.  fast_math: HSG_FLAG_FAST_MATH.  mode: 0 = asynchronous copies land when issued, 1 = when waited for.
 extern "C" int EMU_CAT(emu_zmarch_l, EMU_L)(int G, int mode, int D, int O, int T, const float* temps, unsigned long long seed,
                                              unsigned long long sample_offset, unsigned long long k_hb, int n_or, int n_hb,
-                                             const float* J, const float* H, float* S, double* E, double* M) {
+                                             const float* J, const float* H, float* S, double* E, double* M, int fast_math) {
   constexpr int L = EMU_L;
   Geom g{};
   g.L = L; g.Lh = L / 2; g.ys = L == 64 ? 16 : L; g.D = D; g.O = O; g.T = T; g.R = D * O * T; g.N = (long long)L * L * L;
@@ -90,7 +93,7 @@ extern "C" int EMU_CAT(emu_zmarch_l, EMU_L)(int G, int mode, int D, int O, int T
   convert(true);
   std::vector<double> e_slot(g.R, 0.0), m_slot((size_t)3 * g.R, 0.0);
   ZmarchArgs a{g, priv.data(), jh.data(), temp_of_slot.data(), beta.data(), PhiloxKey{(uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32)},
-               k_hb, n_or, n_hb, E ? e_slot.data() : nullptr, m_slot.data(), 0};
+               k_hb, n_or, n_hb, E ? e_slot.data() : nullptr, m_slot.data(), fast_math};
   emu::mode = mode;
   hsg::seed_jitter = 0;      // exact reciprocal seeds (the variable is shared with any other host build loaded in this process)
   const int rc = dispatch<L>(G, a);

@@ -61,7 +61,7 @@ def _entry(so: Path, L):
     lib = C.CDLL(str(so))
     f = getattr(lib, f"emu_zmarch_l{L}")
     vp, ull, i32 = C.c_void_p, C.c_ulonglong, C.c_int
-    f.argtypes = [i32, i32, i32, i32, i32, vp, ull, ull, ull, i32, i32, vp, vp, vp, vp, vp]
+    f.argtypes = [i32, i32, i32, i32, i32, vp, ull, ull, ull, i32, i32, vp, vp, vp, vp, vp, i32]
     f.restype = i32
     return f
 
@@ -89,7 +89,7 @@ def _run(entry, L, G, mode, D, O, T, calls, seed=5, sample_offset=0, h_r=0.1, t_
     E = np.zeros(D * O * T); M = np.zeros((D * O * T, 3))
     k_hb = 0
     for n_or, n_hb in calls:
-        rc = entry(G, mode, D, O, T, _p(temps), seed, sample_offset, k_hb, n_or, n_hb, _p(J), _p(H), _p(S), _p(E), _p(M))
+        rc = entry(G, mode, D, O, T, _p(temps), seed, sample_offset, k_hb, n_or, n_hb, _p(J), _p(H), _p(S), _p(E), _p(M), 0)
         assert rc == 0, rc
         k_hb += n_hb
         orc.sweep(n_or, n_hb)
@@ -126,6 +126,39 @@ def test_zero_field_and_hot_ladder_on_the_host_model(emu):
     """H = NULL packs as a zero field; a hot ladder drives the heat bath through the series branch (a < 1e-4)."""
     assert _run(emu[16], 16, 2, LATE, 1, 2, 2, [(1, 2)], h_r=0.0) == 0.0
     assert _run(emu[8], 8, 2, EARLY, 1, 2, 2, [(1, 2)], t_lo=1e2, t_hi=1e6) == 0.0
+
+
+@pytest.mark.parametrize("L,G", [(8, 2), (32, 2), (64, 2)])
+def test_fast_math_variant_of_the_sweep_kernel_on_the_host_model(emu, L, G):
+    """zmarch_kernel<..., FM = true> (HSG_FLAG_FAST_MATH), special-function unit modelled by libm: over-relaxation sweeps stay
+    bit-identical, and after one heat-bath sweep colour 0 (drawn from equal inputs) is inside the variant's stated bound,
+    the typical deviation at the 1e-6 level (the same assertions tests/test_variants_gpu.py makes on the GPU)."""
+    from tests.test_device_math_on_host import fast_math_bound
+    D, O, seed = 1, 2, 91
+    temps = np.asarray([0.06, 3.0], dtype=np.float32)
+    T = len(temps)
+    J = hsg_inputs.couplings(L, D, seed); H = hsg_inputs.gaussian_field(L, D, 0.1, seed)
+    orc = oracle.Oracle(L, D, O, temps, seed, precision=32, n_threads=8)
+    orc.set_disorder(J, H); orc.init_spins()
+    S = np.ascontiguousarray(orc.get_spins().astype(np.float32))
+    E = np.zeros(D * O * T); M = np.zeros((D * O * T, 3))
+    assert emu[L](G, LATE, D, O, T, _p(temps), seed, 0, 0, 2, 0, _p(J), _p(H), _p(S), _p(E), _p(M), 1) == 0
+    orc.sweep(2, 0)
+    S1 = orc.get_spins()
+    assert np.array_equal(S.astype(np.float64), S1)
+    assert emu[L](G, EARLY, D, O, T, _p(temps), seed, 0, 0, 0, 1, _p(J), _p(H), _p(S), _p(E), _p(M), 1) == 0
+    orc.sweep(0, 1)
+    dev = np.abs(S.astype(np.float64) - orc.get_spins()).max(axis=3)[0]
+    h = np.broadcast_to(H[0].astype(np.float64), S1[0].shape).copy()
+    for d, ax in enumerate((-1, -2, -3)):
+        h += J[0, d].astype(np.float64) * np.roll(S1[0], -1, axis=ax) + np.roll(J[0, d].astype(np.float64), 1, axis=ax) * np.roll(S1[0], 1, axis=ax)
+    beta = (1.0 / temps.astype(np.float64)).astype(np.float32).astype(np.float64)
+    a = np.sqrt((h ** 2).sum(axis=-4)) * beta[None, :, None, None, None]
+    z, y, x = np.meshgrid(np.arange(L), np.arange(L), np.arange(L), indexing="ij")
+    even = np.broadcast_to((x + y + z) % 2 == 0, dev.shape)
+    assert (dev[even] <= fast_math_bound(a[even]) + 1e-7).all()
+    assert 0 < dev.max() and np.median(dev) < 5e-6 and np.quantile(dev, 0.99) < 2e-4
+    np.testing.assert_allclose(E, orc.energy().reshape(-1), rtol=1e-4)
 
 
 # Seeded faults: the model must SEE a broken protocol, each in the mode its kind of hazard belongs to.
