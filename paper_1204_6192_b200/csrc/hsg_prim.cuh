@@ -39,7 +39,7 @@ __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.app
 
 // special-function unit approximations of the fast-math heat-bath VARIANT only (HSG_FLAG_FAST_MATH, hb_draw_fast): PTX ISA
 // error bounds — ex2: 2^-22 relative; lg2: 2^-22 absolute for arguments in (0.5, 2), 2^-22 relative otherwise;
-// sin, cos: 2^-20.5 absolute on [-2 pi, 2 pi]; sqrt: 2^-23 relative
+// sin, cos: 2^-20.5 absolute on [-pi, pi] (hb_draw_fast keeps the argument there); sqrt: 2^-23 relative
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2_approx(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float sin_approx(float x) { float y; asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
