@@ -151,10 +151,10 @@ def test_start_spins_layout_conversion_and_generic_sweeps_bit_for_bit(lib, L, D,
 
 
 def test_parallel_tempering_observables_and_diagnostics_in_lockstep(lib):
-    L, D, O, T = 4, 2, 3, 5
+    L, D, O, T = 4, 1, 3, 5
     dev, orc, _, _ = _pair(lib, L, D, O, T, seed=21, warm=True)
     n_acc = 0
-    for step in range(40):
+    for step in range(24):
         if step == 5:
             dev.diag_reset(); orc.pt_diag_reset()          # the reset must read the CURRENT (scrambled) permutation
         dev.sweep(1, 1); orc.sweep(1, 1)
@@ -169,10 +169,10 @@ def test_parallel_tempering_observables_and_diagnostics_in_lockstep(lib):
             np.testing.assert_allclose(q0, q0o, rtol=0, atol=1e-13)
             np.testing.assert_allclose(qk, qko, rtol=0, atol=1e-13)
             assert np.abs(E - orc.energy_plain()).max() < L ** 3 / 2 * 9 * 2.0 ** -24 * 8
-    assert n_acc > 20 and not np.array_equal(dev.perm(), np.broadcast_to(np.arange(T), (D, O, T)))
+    assert n_acc > 10 and not np.array_equal(dev.perm(), np.broadcast_to(np.arange(T), (D, O, T)))
     assert np.array_equal(dev.get_spins(), orc.get_spins())
     moved, trav, n, p = dev.diag_get(); m_o, t_o, n_o, p_o = orc.pt_diag_get()
-    assert n == n_o == 35 and np.array_equal(moved, m_o) and np.array_equal(trav, t_o) and trav.sum() > 0
+    assert n == n_o == 19 and np.array_equal(moved, m_o) and np.array_equal(trav, t_o) and trav.sum() > 0
     np.testing.assert_allclose(p, p_o, rtol=1e-15)
 
 
