@@ -198,7 +198,8 @@ const char* hsg_last_sweep_kernel(const hsg_ctx* ctx);
 
 /* Test hook: compares the kernels' branch-free IEEE division / square root with the
  * compiler's correctly rounded ones on n pseudo-random operand sets; counts_dev[0] = division mismatches,
- * counts_dev[1] = square-root mismatches (device memory, 2 x uint64, zeroed by the call). */
+ * counts_dev[1] = square-root mismatches, counts_dev[2] = division mismatches on divisors whose mantissa is all ones (the
+ * one exceptional case of the Newton scheme, counted apart) (device memory, 3 x uint64, zeroed by the call). */
 int hsg_selftest_arith(void* cuda_stream, uint64_t seed, uint64_t n, unsigned long long* counts_dev);
 
 const char* hsg_last_error(const hsg_ctx* ctx);

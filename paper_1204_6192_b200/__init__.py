@@ -86,14 +86,16 @@ def hsg_version() -> str:
     return lib().hsg_version().decode()
 
 
-def hsg_selftest_arith(n, seed=1):
-    """(division mismatches, square-root mismatches) of the kernels' branch-free IEEE routines over n operand sets."""
+def hsg_selftest_arith(n, seed=1, exceptional=False):
+    """(division mismatches, square-root mismatches) of the kernels' branch-free IEEE routines over n operand sets;
+    exceptional=True: the count for divisors whose mantissa is all ones instead (counted apart by the kernel)."""
     import torch
-    counts = torch.zeros(2, dtype=torch.int64, device="cuda")
+    counts = torch.zeros(3, dtype=torch.int64, device="cuda")
     rc = lib().hsg_selftest_arith(C.c_void_p(torch.cuda.current_stream().cuda_stream), int(seed), int(n), counts.data_ptr())
     if rc != HSG_OK:
         raise HsgError(rc, "hsg_selftest_arith failed")
-    return tuple(int(x) for x in counts.cpu())
+    c = tuple(int(x) for x in counts.cpu())
+    return c[2] if exceptional else c[:2]
 
 
 def hsg_xi_second_moment(chi_0, chi_kmin, L) -> float:

@@ -442,7 +442,7 @@ int hsg_pt_diag_get(hsg_ctx* ctx, int64_t* moved_dev, int64_t* traversals_dev, d
 int hsg_selftest_arith(void* cuda_stream, uint64_t seed, uint64_t n, unsigned long long* counts_dev) {
   if (!counts_dev) return HSG_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (cudaMemsetAsync(counts_dev, 0, 2 * sizeof(unsigned long long), st) != cudaSuccess) return HSG_ECUDA;
+  if (cudaMemsetAsync(counts_dev, 0, 3 * sizeof(unsigned long long), st) != cudaSuccess) return HSG_ECUDA;
   PhiloxKey key{(uint32_t)seed, (uint32_t)(seed >> 32)};
   selftest_arith_kernel<<<148 * 8, kThreads, 0, st>>>(key, n, counts_dev);
   return cudaGetLastError() == cudaSuccess ? HSG_OK : HSG_ECUDA;

@@ -480,11 +480,12 @@ __global__ void finalize_overlap_kernel(Geom g, int n_sys /*D*P*T*/, int n_chunk
 // ------------------------------------------------------------------ arithmetic self-test (hsg_selftest_arith)
 // Compares div_rn / sqrt_rn with the compiler's IEEE __fdiv_rn / __fsqrt_rn on pseudo-random operands whose
 // exponents cover [2^-100, 2^100] (all mantissa bits random); counts[0] = division mismatches,
-// counts[1] = square-root mismatches.
+// counts[1] = square-root mismatches, counts[2] = division mismatches on divisors whose mantissa is all ones (counted apart:
+// the one exceptional case of the Newton scheme, see below).
 __global__ void selftest_arith_kernel(PhiloxKey key, unsigned long long n, unsigned long long* __restrict__ counts) {
   const unsigned long long tid = (unsigned long long)blockIdx.x * kThreads + threadIdx.x;
   const unsigned long long stride = (unsigned long long)gridDim.x * kThreads;
-  unsigned int bad_div = 0, bad_sqrt = 0;
+  unsigned int bad_div = 0, bad_sqrt = 0, bad_exc = 0;
   for (unsigned long long i = tid; i < n; i += stride) {
     uint32_t w0, w1, w2, w3;
     philox4x32_10((uint32_t)i, (uint32_t)(i >> 32), 0x5e1f7e57u, 0u, key.k0, key.k1, w0, w1, w2, w3);
@@ -507,10 +508,10 @@ __global__ void selftest_arith_kernel(PhiloxKey key, unsigned long long n, unsig
     // on the rounded quotient only for a good enough seed (tests/test_device_math_on_host.py) — the hardware's must be
     const float b3 = __uint_as_float(__float_as_uint(b) | 0x007FFFFFu), x3 = fabsf(b3);
     const float q3 = __fdiv_rn(a, b3);
-    if (fabsf(q3) >= 1.2e-38f && fabsf(q3) <= 3.0e38f && __float_as_uint(div_rn(a, b3)) != __float_as_uint(q3)) ++bad_div;
-    if (__float_as_uint(rcp_rn<float, false>(x3)) != __float_as_uint(__fdiv_rn(1.0f, x3))) ++bad_div;
-    if (__float_as_uint(div_rn(a2, 1.99999988079071044921875f)) != __float_as_uint(__fdiv_rn(a2, 1.99999988079071044921875f))) ++bad_div;
-    if ((i & 0xFFFFull) == 0 && __float_as_uint(rcp_rn<float, true>(1.99999988079071044921875f)) != 0xBF000001u) ++bad_div;   // -1/(2 - 2^-23)
+    if (fabsf(q3) >= 1.2e-38f && fabsf(q3) <= 3.0e38f && __float_as_uint(div_rn(a, b3)) != __float_as_uint(q3)) ++bad_exc;
+    if (__float_as_uint(rcp_rn<float, false>(x3)) != __float_as_uint(__fdiv_rn(1.0f, x3))) ++bad_exc;
+    if (__float_as_uint(div_rn(a2, 1.99999988079071044921875f)) != __float_as_uint(__fdiv_rn(a2, 1.99999988079071044921875f))) ++bad_exc;
+    if ((i & 0xFFFFull) == 0 && __float_as_uint(rcp_rn<float, true>(1.99999988079071044921875f)) != 0xBF000001u) ++bad_exc;   // -1/(2 - 2^-23)
     const F2 qp = div_rn(make_f2(a, a2), make_f2(b, b2));
     if (fabsf(q2) >= 1.2e-38f && fabsf(q2) <= 3.0e38f && __float_as_uint(f2_lo(qp)) != __float_as_uint(q2)) ++bad_div;
     if (__float_as_uint(f2_hi(qp)) != __float_as_uint(__fdiv_rn(a2, b2))) ++bad_div;
@@ -519,6 +520,7 @@ __global__ void selftest_arith_kernel(PhiloxKey key, unsigned long long n, unsig
   }
   if (bad_div) atomicAdd(counts, (unsigned long long)bad_div);
   if (bad_sqrt) atomicAdd(counts + 1, (unsigned long long)bad_sqrt);
+  if (bad_exc) atomicAdd(counts + 2, (unsigned long long)bad_exc);
 }
 
 }  // namespace hsg

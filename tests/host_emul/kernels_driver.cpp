@@ -200,7 +200,7 @@ unsigned long long emuk_diag_get(void* h, long long* moved, long long* trav, dou
 
 // hsg_selftest_arith on the host (IEEE division / square root of the host as the reference)
 void emuk_selftest(unsigned long long seed, unsigned long long n, unsigned long long* counts) {
-  counts[0] = counts[1] = 0;
+  counts[0] = counts[1] = counts[2] = 0;
   hsg::seed_jitter = 0;
   PhiloxKey key{(uint32_t)seed, (uint32_t)(seed >> 32)};
   serial_grid(4, kThreads, [&] { selftest_arith_kernel(key, n, counts); });
