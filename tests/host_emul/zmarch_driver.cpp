@@ -43,6 +43,7 @@ int dispatch(int G, const ZmarchArgs& a) {
     case 1: sweep<L, 1>(a); return 0;
     case 2: sweep<L, 2>(a); return 0;
 #if EMU_L == 8 || EMU_L == 16
+    case 4: sweep<L, 4>(a); return 0;
     case 8: sweep<L, 8>(a); return 0;
 #endif
     default: return -1;

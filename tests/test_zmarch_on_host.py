@@ -107,8 +107,10 @@ CASES = [
     (8, 2, 2, 2, 3, [(2, 1), (1, 2)]),
     (8, 8, 1, 2, 4, [(1, 1)]),
     (8, 1, 1, 1, 3, [(1, 1)]),               # 16-thread CTA (O*T odd): half a warp
+    (8, 4, 1, 2, 2, [(1, 1)]),               # the group size zmarch_pick_g takes for a few hundred systems
     (16, 1, 1, 1, 3, [(2, 1)]),
     (16, 8, 2, 2, 4, [(2, 0), (0, 2)]),
+    (16, 4, 1, 2, 2, [(1, 1)]),
     (32, 2, 1, 2, 2, [(2, 1)]),
     (32, 1, 1, 1, 1, [(1, 1)]),
     (64, 2, 1, 2, 1, [(1, 1)]),              # thread-block cluster of four strips, two systems per CTA
