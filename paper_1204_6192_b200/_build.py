@@ -1,11 +1,13 @@
 """In-tree build of the C-ABI library ``lib/libhsg.so`` (CUDA, sm_100a only).
 
 ``nvcc`` cross-compiles without a GPU (one translation unit per lattice size of the sweep kernel, compiled in parallel), so this runs on the CPU box (``__graft_entry__.build()``) and on
-the GPU box alike.  The shared object is rebuilt when any source under ``csrc/`` or ``include/hsg.h``
-is newer than it.
+the GPU box alike.  The shared object is rebuilt when the contents of any source under ``csrc/`` or of
+``include/hsg.h`` (or the compiler flags) differ from what it was built from: a digest kept beside it, not file
+times, so that a copy of the tree whose times were not preserved is not rebuilt.
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import re
 import shutil
@@ -17,6 +19,7 @@ _ROOT = _PKG.parent
 CSRC = _PKG / "csrc"
 HEADER = _ROOT / "include" / "hsg.h"
 LIB = _PKG / "lib" / "libhsg.so"
+DIGEST = _PKG / "lib" / "libhsg.sources.sha256"
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -37,11 +40,17 @@ def sources():
     return sorted(CSRC.glob("*.cu")) + sorted(CSRC.glob("*.cuh")) + sorted(CSRC.glob("*.h")) + [HEADER]
 
 
+def _digest() -> str:
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for p in sources():
+        h.update(p.name.encode()); h.update(b"\0"); h.update(p.read_bytes()); h.update(b"\0")
+    return h.hexdigest()
+
+
 def stale() -> bool:
-    if not LIB.exists():
+    if not LIB.exists() or not DIGEST.exists():
         return True
-    t = LIB.stat().st_mtime
-    return any(p.stat().st_mtime > t for p in sources())
+    return DIGEST.read_text().strip() != _digest()
 
 
 def _deps(unit: Path) -> set:
@@ -57,6 +66,18 @@ def _deps(unit: Path) -> set:
     return seen
 
 
+def _unit_digest(unit: Path) -> str:
+    """Digest of a translation unit: the compiler flags and the contents of every file it includes."""
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for p in sorted(_deps(unit)):
+        h.update(p.name.encode()); h.update(b"\0"); h.update(p.read_bytes()); h.update(b"\0")
+    return h.hexdigest()
+
+
+def _unit_digest_file(obj: Path) -> Path:
+    return obj.with_suffix(".sha256")
+
+
 def build(force: bool = False, verbose: bool = False) -> Path:
     """Compile the translation units under csrc/ whose sources changed (in parallel; objects are kept under lib/obj/) and
     link lib/libhsg.so; returns its path.  Fails loudly: there is no CPU fallback."""
@@ -66,14 +87,11 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     objdir.mkdir(parents=True, exist_ok=True)
     nvcc = _nvcc()
     units = sorted(CSRC.glob("*.cu"))
-    flag_tag = " ".join(NVCC_FLAGS)
-    tag_file = objdir / "flags.txt"
-    if not tag_file.exists() or tag_file.read_text() != flag_tag:
-        force = True
     todo = []
     for u in units:
         o = objdir / (u.stem + ".o")
-        if force or not o.exists() or any(d.stat().st_mtime > o.stat().st_mtime for d in _deps(u)):
+        d = _unit_digest_file(o)
+        if force or not o.exists() or not d.exists() or d.read_text().strip() != _unit_digest(u):
             todo.append((u, o))
     cmds = [[nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", str(u), "-o", str(o)] for u, o in todo]
     procs = [subprocess.Popen(c, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True) for c in cmds]
@@ -83,7 +101,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
             raise RuntimeError("nvcc failed:\n" + " ".join(c) + "\n" + o)
         if verbose:
             print(o)
-    tag_file.write_text(flag_tag)
+    for u, o in todo:
+        _unit_digest_file(o).write_text(_unit_digest(u))
     tmp = LIB.with_name(f"libhsg.tmp{os.getpid()}.so")
     link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler", "-fPIC",
             *[str(objdir / (u.stem + ".o")) for u in units], "-o", str(tmp)]
@@ -91,6 +110,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if res.returncode != 0:
         raise RuntimeError("link failed:\n" + " ".join(link) + "\n" + res.stdout + res.stderr)
     os.replace(tmp, LIB)
+    DIGEST.write_text(_digest())
     return LIB
 
 
