@@ -164,7 +164,14 @@ def test_two_gpu_processes_gathered_over_gloo_reproduce_one_context():
     procs = [ctx.Process(target=_gpu_worker, args=(r, 2, port, q, n_all)) for r in range(2)]
     for p in procs:
         p.start()
-    got = q.get(timeout=600)
+    got, waited = None, 0
+    while got is None:                       # fail at once if a rank dies, not after the queue's time-out
+        try:
+            got = q.get(timeout=5)
+        except Exception:
+            waited += 5
+            assert all(p.exitcode in (None, 0) for p in procs), [p.exitcode for p in procs]
+            assert waited < 600, "ranks still running after 600 s"
     for p in procs:
         p.join(timeout=120)
         assert p.exitcode == 0
