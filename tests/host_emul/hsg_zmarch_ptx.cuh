@@ -54,6 +54,7 @@ template <int V> inline void sts(uint32_t a, const F2 (&r)[V / 2]) {
 }
 // st.async: remote store whose bytes are counted on an mbarrier of the destination CTA
 template <int V> inline void st_async(uint32_t a, const F2 (&r)[V / 2], uint32_t bar) {
+  if ((a & 0xFFFFFFu) % (4u * V) || (bar & 7u)) { std::fprintf(stderr, "emu: misaligned st.async or mbarrier\n"); std::abort(); }
   emu::Copy c{emu::ptr_of(a), nullptr, 4u * V, {0}, true};
   std::memcpy(c.imm, &r[0], 4u * V);
   emu::cta_of(bar)->mbar(bar & 0xFFFFFFu).transfer(c);
