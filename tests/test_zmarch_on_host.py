@@ -112,7 +112,7 @@ CASES = [
     (16, 8, 2, 2, 4, [(2, 0), (0, 2)]),
     (16, 4, 1, 2, 2, [(1, 1)]),
     (32, 2, 1, 2, 2, [(2, 1)]),
-    (32, 1, 1, 1, 1, [(1, 1)]),
+    (32, 1, 2, 1, 1, [(1, 1)]),              # two samples: the J/H planes of the second one
     (64, 2, 1, 2, 1, [(1, 1)]),              # thread-block cluster of four strips, two systems per CTA
     (64, 1, 1, 1, 1, [(1, 1)]),
 ]
