@@ -81,8 +81,9 @@ def _run(prog, *args, env=ENV):
 
 
 # (L, G, D, O, T, n_or, n_hb): several warps per CTA wherever the size allows, several samples, both kinds of sweep
-CASES = [(8, 8, 1, 2, 4, 1, 1), (8, 1, 1, 1, 3, 1, 1), (16, 8, 2, 2, 4, 1, 1), (16, 4, 1, 2, 2, 1, 1),
-         (32, 2, 2, 2, 1, 1, 1), (64, 2, 1, 2, 1, 1, 1)]
+# (several sweeps per launch at the small sizes: the rings run on across the sweeps of a call)
+CASES = [(8, 8, 1, 2, 4, 3, 2), (8, 1, 1, 1, 3, 1, 1), (16, 8, 1, 2, 4, 2, 1), (16, 4, 1, 2, 2, 1, 1),
+         (32, 2, 1, 2, 1, 2, 1), (64, 1, 1, 1, 1, 1, 1)]
 RUNS = [("thread", c) for c in CASES] + [("address", c) for c in CASES if c[0] in ASAN_SIZES and c[1] != 4]
 
 
